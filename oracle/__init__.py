@@ -1,0 +1,151 @@
+"""CPU oracle for the hot path of arXiv 1306.5076 -- TEST INFRASTRUCTURE, not the product.
+
+Thin ctypes wrapper over oracle/libbcf_oracle.so (plain C, see bcf_oracle_impl.h for the
+arithmetic and its PAPER.md citations).  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this package; the CUDA path
+(paper_1306_5076_b200) never does, and this package never imports it.
+
+All functions take numpy arrays (keys: uint32 or uint64; vals: uint32 or None), leave their
+inputs untouched and return new arrays.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        path = _build.build()
+        lib = ctypes.CDLL(path)
+        vp, sz, ci = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int
+        for s in ("k32", "k64"):
+            getattr(lib, f"bcf_oracle_shearsort_tiles_{s}").argtypes = [vp, vp, sz, sz, ci, ci]
+            getattr(lib, f"bcf_oracle_merge_two_{s}").argtypes = [vp, vp, sz, vp, vp, sz, vp, vp]
+            getattr(lib, f"bcf_oracle_merge_runs_{s}").argtypes = [vp, vp, sz, sz]
+            getattr(lib, f"bcf_oracle_sort_full_{s}").argtypes = [vp, vp, sz, sz]
+            getattr(lib, f"bcf_oracle_corank_{s}").argtypes = [vp, vp, sz, vp, vp, sz, sz]
+            getattr(lib, f"bcf_oracle_corank_{s}").restype = sz
+            getattr(lib, f"bcf_oracle_shearsort_merge_{s}").argtypes = [vp, vp, sz, sz]
+            getattr(lib, f"bcf_oracle_binary_merge_pagewise_{s}").argtypes = [vp, vp, sz, vp, vp, sz, vp, vp, sz]
+        _LIB = lib
+    return _LIB
+
+
+def _suffix(keys):
+    if keys.dtype == np.uint32:
+        return "k32"
+    if keys.dtype == np.uint64:
+        return "k64"
+    raise TypeError(f"keys must be uint32 or uint64, got {keys.dtype}")
+
+
+def _prep(keys, vals, copy=True):
+    k = np.array(keys, copy=True) if copy else np.ascontiguousarray(keys)
+    k = np.ascontiguousarray(k)
+    _suffix(k)
+    v = None
+    if vals is not None:
+        v = np.array(vals, dtype=np.uint32, copy=True) if copy else np.ascontiguousarray(vals, dtype=np.uint32)
+        if v.shape != k.shape:
+            raise ValueError("keys and vals must have the same shape")
+    return k, v
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _ret(k, v):
+    return k if v is None else (k, v)
+
+
+def _check(rc, what):
+    if rc < 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+    return rc
+
+
+def shearsort_tiles(keys, vals=None, w=32, final_snake=False, phases=-1):
+    """ShearSort (Alg. 1) each consecutive row-major w*w tile of a flat array."""
+    k, v = _prep(keys, vals)
+    k = k.reshape(-1)
+    if v is not None:
+        v = v.reshape(-1)
+    if w <= 0 or k.size % (w * w):
+        raise ValueError("size must be a multiple of w*w")
+    fn = getattr(_lib(), f"bcf_oracle_shearsort_tiles_{_suffix(k)}")
+    _check(fn(_p(k), _p(v), k.size // (w * w), w, int(bool(final_snake)), int(phases)), "shearsort_tiles")
+    return _ret(k, v)
+
+
+def merge_two(ka, kb, va=None, vb=None):
+    """Two-finger merge of two sorted sequences, ties from A."""
+    a, av = _prep(ka, va, copy=False)
+    b, bv = _prep(kb, vb, copy=False)
+    if a.dtype != b.dtype or (av is None) != (bv is None):
+        raise TypeError("A and B must have the same element type")
+    ko = np.empty(a.size + b.size, dtype=a.dtype)
+    vo = None if av is None else np.empty(a.size + b.size, dtype=np.uint32)
+    fn = getattr(_lib(), f"bcf_oracle_merge_two_{_suffix(a)}")
+    _check(fn(_p(a), _p(av), a.size, _p(b), _p(bv), b.size, _p(ko), _p(vo)), "merge_two")
+    return _ret(ko, vo)
+
+
+def merge_runs(keys, run_len, vals=None, return_rounds=False):
+    """Pairwise merge rounds over sorted runs of run_len."""
+    k, v = _prep(keys, vals)
+    fn = getattr(_lib(), f"bcf_oracle_merge_runs_{_suffix(k)}")
+    rounds = _check(fn(_p(k), _p(v), k.size, int(run_len)), "merge_runs")
+    out = _ret(k, v)
+    return (out, rounds) if return_rounds else out
+
+
+def sort_full(keys, vals=None, w=32, return_rounds=False):
+    """BCFMergesort: ShearSort base case on w*w tiles + merge rounds (section 3)."""
+    k, v = _prep(keys, vals)
+    fn = getattr(_lib(), f"bcf_oracle_sort_full_{_suffix(k)}")
+    rounds = _check(fn(_p(k), _p(v), k.size, int(w)), "sort_full")
+    out = _ret(k, v)
+    return (out, rounds) if return_rounds else out
+
+
+def corank(ka, kb, d, va=None, vb=None):
+    """Number of elements the A-first two-finger merge takes from A for its first d outputs."""
+    a, av = _prep(ka, va, copy=False)
+    b, bv = _prep(kb, vb, copy=False)
+    if a.dtype != b.dtype or (av is None) != (bv is None):
+        raise TypeError("A and B must have the same element type")
+    fn = getattr(_lib(), f"bcf_oracle_corank_{_suffix(a)}")
+    r = fn(_p(a), _p(av), a.size, _p(b), _p(bv), b.size, int(d))
+    if r == ctypes.c_size_t(-1).value:
+        raise RuntimeError("oracle corank failed")
+    return int(r)
+
+
+def shearsort_merge(keys, na, vals=None, w=32):
+    """SHEARSORT-MERGE on one page of w*w elements: [0,na) and [na,w*w) sorted (A8)."""
+    k, v = _prep(keys, vals)
+    if k.size != w * w:
+        raise ValueError("page must hold w*w elements")
+    fn = getattr(_lib(), f"bcf_oracle_shearsort_merge_{_suffix(k)}")
+    _check(fn(_p(k), _p(v), int(w), int(na)), "shearsort_merge")
+    return _ret(k, v)
+
+
+def binary_merge_pagewise(ka, kb, va=None, vb=None, w=32):
+    """BINARY-MERGE, the page-wise streaming merge of PAPER.md Alg. 6 with M = w*w."""
+    a, av = _prep(ka, va, copy=False)
+    b, bv = _prep(kb, vb, copy=False)
+    if a.dtype != b.dtype or (av is None) != (bv is None):
+        raise TypeError("A and B must have the same element type")
+    ko = np.empty(a.size + b.size, dtype=a.dtype)
+    vo = None if av is None else np.empty(a.size + b.size, dtype=np.uint32)
+    fn = getattr(_lib(), f"bcf_oracle_binary_merge_pagewise_{_suffix(a)}")
+    _check(fn(_p(a), _p(av), a.size, _p(b), _p(bv), b.size, _p(ko), _p(vo), int(w)), "binary_merge_pagewise")
+    return _ret(ko, vo)

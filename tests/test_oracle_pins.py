@@ -1,0 +1,321 @@
+"""Pins for the CPU oracle (oracle/): what the paper and the mathematics fix, none of it the oracle
+re-typed.  SURVEY.md section 8c lists them; each test names the reading (A1..A15) it pins.
+
+ * 0-1 principle, exhaustively
+ * exhaustive permutations / small alphabets against the closed form "sorted order"
+ * the dirty-row halving invariant and the snake order of classic ShearSort
+ * textbook library sorts (numpy) on every config shape
+ * the trace of a stable two-finger merge, written out in Python, for the co-rank
+ * the paper's pass count (Lemma 2)
+"""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1306_5076_b200 import workloads
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def all_01_matrices(w):
+    m = w * w
+    idx = np.arange(1 << m, dtype=np.uint64)
+    bits = ((idx[:, None] >> np.arange(m, dtype=np.uint64)[None, :]) & np.uint64(1)).astype(np.uint32)
+    return bits  # shape (2^m, m), one row-major tile per row
+
+
+def expected_01(tiles):
+    """Closed form of a sorted 0/1 tile: (#zeros) zeros, then ones."""
+    m = tiles.shape[1]
+    ones = tiles.sum(axis=1)
+    return (np.arange(m)[None, :] >= (m - ones)[:, None]).astype(np.uint32)
+
+
+# ---------------------------------------------------------------- ShearSort (Alg. 1), A1-A4
+
+
+@pytest.mark.parametrize("w", [1, 2, 3, 4])
+def test_shearsort_sorts_every_01_matrix(w):
+    tiles = all_01_matrices(w)
+    out = oracle.shearsort_tiles(tiles.reshape(-1), w=w).reshape(tiles.shape)
+    assert np.array_equal(out, expected_01(tiles))
+
+
+def test_shearsort_one_phase_fewer_fails():
+    """A2: ceil(log2 w) phases are necessary: with one fewer, w = 4 fails (mutation pin)."""
+    tiles = all_01_matrices(4)
+    out = oracle.shearsort_tiles(tiles.reshape(-1), w=4, phases=1).reshape(tiles.shape)
+    bad = int((out != expected_01(tiles)).any(axis=1).sum())
+    assert bad > 0
+    assert bad == 17696  # an independent check found the same count
+
+
+@pytest.mark.parametrize("w", [2, 3, 4])
+def test_shearsort_classic_snake_order(w):
+    """A4: with an alternating final row pass the tile is in snake order (Sen et al.)."""
+    tiles = all_01_matrices(w)
+    out = oracle.shearsort_tiles(tiles.reshape(-1), w=w, final_snake=True).reshape(-1, w, w)
+    snake = out.copy()
+    snake[:, 1::2, :] = snake[:, 1::2, ::-1]
+    assert np.array_equal(snake.reshape(tiles.shape), expected_01(tiles))
+
+
+@pytest.mark.parametrize("w", [8, 16, 32])
+def test_shearsort_dirty_rows_halve(w):
+    """0-1 argument behind L109: after k phases at most ceil(w / 2^k) rows are dirty."""
+    rng = np.random.default_rng(1234 + w)
+    num = 64
+    dens = rng.random((num, 1, 1))
+    tiles = (rng.random((num, w, w)) < dens).astype(np.uint32)
+    # structured worst-ish cases: staircase and checkerboard
+    tiles[0] = (np.add.outer(np.arange(w), np.arange(w)) % 2).astype(np.uint32)
+    tiles[1] = (np.arange(w)[:, None] > np.arange(w)[None, :]).astype(np.uint32)
+    for k in range(0, int(math.log2(w)) + 1):
+        out = oracle.shearsort_tiles(tiles.reshape(-1), w=w, phases=k).reshape(num, w, w)
+        rowsum = out.sum(axis=2)
+        dirty = ((rowsum != 0) & (rowsum != w)).sum(axis=1)
+        assert dirty.max() <= math.ceil(w / 2 ** k)
+    final = oracle.shearsort_tiles(tiles.reshape(-1), w=w).reshape(num, -1)
+    assert np.array_equal(final, expected_01(tiles.reshape(num, -1)))
+
+
+@pytest.mark.parametrize("w", [2, 3, 5, 8, 32])
+def test_shearsort_random_vs_library_sort(w):
+    rng = np.random.default_rng(99 + w)
+    x = rng.integers(0, 1 << 32, size=(37, w * w), dtype=np.uint64).astype(np.uint32)
+    x[3] = 7  # all equal
+    x[4] = np.arange(w * w, dtype=np.uint32)[::-1]
+    x[5, : w * w // 2] = 0xFFFFFFFF  # the padding value is a legal key (A10)
+    out = oracle.shearsort_tiles(x.reshape(-1), w=w).reshape(x.shape)
+    assert np.array_equal(out, np.sort(x, axis=1))
+
+
+def test_shearsort_key_value_lexicographic():
+    """A11: order is (key, value) lexicographic; with value = index it equals a stable sort."""
+    k, v = workloads.cfg2_tiles_u32_u32(num_tiles=5)
+    ko, vo = oracle.shearsort_tiles(k, v)
+    for t in range(5):
+        s = slice(t * 1024, (t + 1) * 1024)
+        order = np.argsort(k[s], kind="stable")
+        assert np.array_equal(ko[s], k[s][order])
+        assert np.array_equal(vo[s], v[s][order])
+    # scrambled values: plain lexicographic order
+    rng = np.random.default_rng(5)
+    v2 = rng.permutation(v.size).astype(np.uint32)
+    ko, vo = oracle.shearsort_tiles(k[:2048], v2[:2048])
+    for t in range(2):
+        s = slice(t * 1024, (t + 1) * 1024)
+        order = np.lexsort((v2[s], k[s]))
+        assert np.array_equal(ko[s], k[s][order]) and np.array_equal(vo[s], v2[s][order])
+
+
+def test_shearsort_u64_keys():
+    k, v = workloads.cfg5a_sort_u64_u32(n=3 * 1024)
+    ko, vo = oracle.shearsort_tiles(k, v)
+    for t in range(3):
+        s = slice(t * 1024, (t + 1) * 1024)
+        order = np.lexsort((v[s], k[s]))
+        assert np.array_equal(ko[s], k[s][order]) and np.array_equal(vo[s], v[s][order])
+
+
+# ---------------------------------------------------------------- merge (L125), co-rank (A12)
+
+
+def python_merge_trace(a, b):
+    """A stable two-finger merge written out in Python; returns (output, i after d outputs)."""
+    i = j = 0
+    out, trace = [], [0]
+    while i < len(a) or j < len(b):
+        if j >= len(b) or (i < len(a) and a[i] <= b[j]):
+            out.append(a[i]); i += 1
+        else:
+            out.append(b[j]); j += 1
+        trace.append(i)
+    return out, trace
+
+
+def test_merge_two_and_corank_match_stable_merge_trace():
+    rng = np.random.default_rng(7)
+    for case in range(300):
+        na, nb = int(rng.integers(0, 40)), int(rng.integers(0, 40))
+        hi = int(rng.choice([2, 5, 1000]))
+        a = np.sort(rng.integers(0, hi, size=na)).astype(np.uint32)
+        b = np.sort(rng.integers(0, hi, size=nb)).astype(np.uint32)
+        out, trace = python_merge_trace(a.tolist(), b.tolist())
+        assert oracle.merge_two(a, b).tolist() == out
+        for d in range(na + nb + 1):
+            i = oracle.corank(a, b, d)
+            assert i == trace[d]
+            j = d - i
+            assert 0 <= i <= na and 0 <= j <= nb
+            if i > 0 and j < nb:
+                assert a[i - 1] <= b[j]
+            if j > 0 and i < na:
+                assert b[j - 1] < a[i]
+
+
+def test_corank_ties_take_from_A_first():
+    a = np.array([5, 5], dtype=np.uint32)
+    b = np.array([5, 5], dtype=np.uint32)
+    assert [oracle.corank(a, b, d) for d in range(5)] == [0, 1, 2, 2, 2]
+    # with values the tie is broken by value
+    assert oracle.corank(a, b, 2, va=np.array([1, 3], np.uint32), vb=np.array([0, 2], np.uint32)) == 1
+
+
+def test_merge_two_key_value_u64():
+    rng = np.random.default_rng(11)
+    ka = rng.integers(0, 4, size=50, dtype=np.uint64) << np.uint64(40)
+    kb = rng.integers(0, 4, size=70, dtype=np.uint64) << np.uint64(40)
+    va = rng.integers(0, 1 << 32, size=50, dtype=np.uint64).astype(np.uint32)
+    vb = rng.integers(0, 1 << 32, size=70, dtype=np.uint64).astype(np.uint32)
+    oa = np.lexsort((va, ka)); ka, va = ka[oa], va[oa]
+    ob = np.lexsort((vb, kb)); kb, vb = kb[ob], vb[ob]
+    ko, vo = oracle.merge_two(ka, kb, va, vb)
+    k = np.concatenate([ka, kb]); v = np.concatenate([va, vb])
+    o = np.lexsort((v, k))
+    assert np.array_equal(ko, k[o]) and np.array_equal(vo, v[o])
+
+
+# ---------------------------------------------------------------- full sort / merge rounds (L103)
+
+
+def test_sort_full_all_permutations_n_le_8():
+    """Two (or fewer) 2x2 tiles + merge rounds on every permutation of n <= 8 keys."""
+    for n in range(0, 9):
+        want = np.arange(n, dtype=np.uint32)
+        for p in itertools.permutations(range(n)):
+            x = np.array(p, dtype=np.uint32)
+            assert np.array_equal(oracle.sort_full(x, w=2), want)
+
+
+def test_sort_full_all_ternary_words_of_length_8():
+    for word in itertools.product(range(3), repeat=8):
+        x = np.array(word, dtype=np.uint32)
+        assert oracle.sort_full(x, w=2).tolist() == sorted(word)
+
+
+def test_merge_runs_all_sorted_pairs_of_permutations_n8():
+    """merge_runs on every permutation of 8 keys whose runs of length r were pre-sorted."""
+    for r in (1, 2, 3, 4, 5):
+        for p in itertools.islice(itertools.permutations(range(8)), 0, None, 7):
+            x = workloads.sorted_runs(np.array(p, dtype=np.uint32), r)
+            assert np.array_equal(oracle.merge_runs(x, r), np.arange(8, dtype=np.uint32))
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 1023, 1024, 1025, 5000, 3 * 1024 + 17])
+def test_sort_full_ragged_sizes_and_padding_value(n):
+    """A10: partial tiles are padded with all-ones in scratch only; 0xFFFFFFFF is a legal key."""
+    rng = np.random.default_rng(n)
+    x = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(np.uint32)
+    if n > 4:
+        x[:: max(1, n // 5)] = 0xFFFFFFFF
+    out, rounds = oracle.sort_full(x, return_rounds=True)
+    assert np.array_equal(out, np.sort(x))
+    tiles = max(1, math.ceil(n / 1024))
+    assert rounds == math.ceil(math.log2(tiles))  # Lemma 2: 1 + ceil(log2(N/M)) scans
+
+
+def test_sort_full_config_shapes_vs_library_sort():
+    x = workloads.cfg3_sort_u32(n=1 << 14)
+    assert np.array_equal(oracle.sort_full(x), np.sort(x))
+    for dist in workloads.CFG4_VARIANTS:
+        x = workloads.cfg4_sort_u32(dist, n=(1 << 13) + 77)
+        out = oracle.sort_full(x)
+        assert np.array_equal(out, np.sort(x)), dist
+        assert np.all(out[:-1] <= out[1:])
+    k, v = workloads.cfg5a_sort_u64_u32(n=(1 << 13) + 5)
+    ko, vo = oracle.sort_full(k, v)
+    o = np.lexsort((v, k))
+    assert np.array_equal(ko, k[o]) and np.array_equal(vo, v[o])
+    o2 = np.argsort(k, kind="stable")  # value = index  =>  stable sort by key
+    assert np.array_equal(vo, v[o2])
+
+
+@pytest.mark.parametrize("k", [2, 64, 1024])
+def test_merge_runs_config_5b_shape(k):
+    keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=1 << 15)
+    out, rounds = oracle.merge_runs(keys, run_len, return_rounds=True)
+    assert rounds == int(math.log2(k))
+    assert np.array_equal(out, np.sort(keys))
+
+
+def test_merge_runs_ragged_runs():
+    rng = np.random.default_rng(3)
+    for n, r in [(10, 3), (1000, 7), (4097, 1024), (5000, 1), (777, 1000)]:
+        x = rng.integers(0, 50, size=n).astype(np.uint32)
+        xs = workloads.sorted_runs(x, r)
+        assert np.array_equal(oracle.merge_runs(xs, r), np.sort(x))
+
+
+# ---------------------------------------------------------------- SHEARSORT-MERGE (A8), Alg. 6 (A9)
+
+
+def test_a8_contiguous_placement_counterexample():
+    """One ShearSort round on contiguously placed half-pages does not merge (golden fixture)."""
+    rows = {}
+    with open(os.path.join(GOLDEN, "a8_counterexample.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            name, *vals = line.split()
+            rows[name] = np.array(vals, dtype=np.uint32)
+    page = np.concatenate([rows["A"], rows["B"]])
+    out = oracle.shearsort_tiles(page, w=4, phases=1)
+    assert np.array_equal(out, rows["AFTER"])
+    assert not np.array_equal(out, np.sort(page))
+    # the reading adopted (second page reversed, {column sort; row sort}) does merge it
+    assert np.array_equal(oracle.shearsort_merge(page, na=8, w=4), np.sort(page))
+
+
+@pytest.mark.parametrize("w", [2, 4, 8])
+def test_shearsort_merge_every_sorted_01_pair_every_split(w):
+    """0-1 principle for merging networks: all sorted-0/1 (A, B) with |A| + |B| = w^2."""
+    m = w * w
+    for na in range(m + 1):
+        nb = m - na
+        for za in range(na + 1):
+            for zb in range(nb + 1):
+                page = np.concatenate([np.arange(na) >= za, np.arange(nb) >= zb]).astype(np.uint32)
+                out = oracle.shearsort_merge(page, na=na, w=w)
+                assert out.sum() == page.sum() and np.all(out[:-1] <= out[1:]), (na, za, zb)
+
+
+def test_shearsort_merge_random_w32():
+    rng = np.random.default_rng(8)
+    for _ in range(60):
+        na = int(rng.integers(0, 1025))
+        x = rng.integers(0, int(rng.choice([3, 1 << 32])), size=1024, dtype=np.uint64).astype(np.uint32)
+        page = np.concatenate([np.sort(x[:na]), np.sort(x[na:])])
+        assert np.array_equal(oracle.shearsort_merge(page, na=na), np.sort(x))
+
+
+@pytest.mark.parametrize("w", [2, 4, 8, 32])
+def test_binary_merge_pagewise_equals_sorted_union(w):
+    rng = np.random.default_rng(40 + w)
+    m = w * w
+    sizes = [(0, 0), (0, 5), (5, 0), (1, 1), (m // 2, m // 2), (m, m), (3 * m, 3 * m),
+             (m // 2 - 1, 2 * m + 3), (5 * m + 1, 7), (4 * m, m // 2)]
+    sizes += [tuple(int(s) for s in rng.integers(0, 6 * m, size=2)) for _ in range(60)]
+    for na, nb in sizes:
+        hi = int(rng.choice([2, 7, 1 << 32]))
+        a = np.sort(rng.integers(0, hi, size=na, dtype=np.uint64).astype(np.uint32))
+        b = np.sort(rng.integers(0, hi, size=nb, dtype=np.uint64).astype(np.uint32))
+        if na and rng.random() < 0.3:
+            a[-1] = 0xFFFFFFFF  # a real key equal to the padding value
+        out = oracle.binary_merge_pagewise(a, b, w=w)
+        assert np.array_equal(out, np.sort(np.concatenate([a, b]))), (w, na, nb)
+
+
+def test_binary_merge_pagewise_key_value():
+    rng = np.random.default_rng(77)
+    k = rng.integers(0, 9, size=3000, dtype=np.uint64)
+    v = np.arange(3000, dtype=np.uint32)
+    o = np.lexsort((v[:1300], k[:1300])); ka, va = k[:1300][o], v[:1300][o]
+    o = np.lexsort((v[1300:], k[1300:])); kb, vb = k[1300:][o], v[1300:][o]
+    ko, vo = oracle.binary_merge_pagewise(ka, kb, va, vb)
+    o = np.lexsort((v, k))
+    assert np.array_equal(ko, k[o]) and np.array_equal(vo, v[o])
