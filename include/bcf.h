@@ -1,0 +1,232 @@
+/*
+ * bcf.h -- C ABI of the B200-native bank-conflict-free sorting library (libbcf.so).
+ *
+ * The library implements the data-parallel hot path of
+ *   Sitchinava & Weichert, "Bank Conflict Free Comparison-based Sorting On GPUs",
+ *   arXiv 1306.5076 (cited below as PAPER.md:L<line>, section / algorithm),
+ * as hand-written sm_100a CUDA kernels:  the ShearSort of w x w = 32 x 32 tiles in shared
+ * memory (section 3.1, Alg. 1/2) and BCFMergesort's merging of sorted runs larger
+ * than shared memory (section 3, 3.2, Alg. 6).
+ *
+ * Conventions for every entry point
+ *  - Elements are keys alone, or (key, value) pairs in two separate arrays (SoA).
+ *    Supported element types: (U32, NONE), (U32, U32), (U64, NONE), (U64, U32).
+ *  - ORDER: ascending by (key, value) compared lexicographically as unsigned integers; for
+ *    keys-only, by key.  That order is total on element bit patterns, so exactly one output is
+ *    correct for every input (reading A11).
+ *  - POINTERS named d_* are DEVICE pointers, h_* are HOST pointers.  All device arrays must be
+ *    16-byte aligned (BCF_ERR_MISALIGNED otherwise).  d_vals must be NULL iff the value type is
+ *    BCF_VAL_NONE.
+ *  - OWNERSHIP: the caller owns every byte, including the workspace; the library never
+ *    allocates or frees device memory.
+ *  - ASYNCHRONY: device entry points only enqueue work on `stream` and return; they never
+ *    synchronise.  (bcf_sort_host is the exception, see there.)
+ *  - ERRORS: status codes only; no exceptions, no exit().  n == 0 is BCF_OK and a no-op.
+ *    A failed launch returns BCF_ERR_CUDA and leaves cudaGetLastError() for the caller.
+ *  - DEVICE: compute capability 10.x (B200, sm_100a) is required; anything else returns
+ *    BCF_ERR_UNSUPPORTED_DEVICE.  There is no fallback path of any kind.
+ *  - LIMIT: n < 2^32 elements.
+ */
+#ifndef BCF_H_
+#define BCF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BCF_W 32            /* warp size = number of 4-byte shared memory banks */
+#define BCF_TILE 1024       /* M = w*w elements per tile / page           */
+
+/* A CUDA stream handle; identical to cudaStream_t / CUstream. */
+typedef struct CUstream_st *bcf_stream_t;
+
+typedef enum {
+    BCF_OK = 0,
+    BCF_ERR_INVALID_ARG = 1,         /* NULL pointer, bad enum, run_len == 0, in/out aliasing, n >= 2^32 */
+    BCF_ERR_MISALIGNED = 2,          /* a device pointer is not 16-byte aligned                         */
+    BCF_ERR_WORKSPACE_TOO_SMALL = 3, /* workspace_bytes < bcf_workspace_bytes(...)                      */
+    BCF_ERR_UNSUPPORTED_DEVICE = 4,  /* current device is not compute capability 10.x                   */
+    BCF_ERR_CUDA = 5                 /* a CUDA runtime call or kernel launch failed                     */
+} bcf_status;
+
+typedef enum { BCF_KEY_U32 = 0, BCF_KEY_U64 = 1 } bcf_key_t;
+typedef enum { BCF_VAL_NONE = 0, BCF_VAL_U32 = 1 } bcf_val_t;
+
+typedef enum {
+    BCF_OP_SORT_TILES = 0,
+    BCF_OP_MERGE_RUNS = 1,
+    BCF_OP_SORT = 2,
+    BCF_OP_SORT_HOST = 3,
+    BCF_OP_MERGE_PAGEWISE = 4
+} bcf_op_t;
+
+/* Human-readable name of a status code (static storage). */
+const char *bcf_status_string(bcf_status s);
+
+/* Library version, e.g. "bcf 0.1 (sm_100a)". */
+const char *bcf_version(void);
+
+/*
+ * Bytes of device workspace the given operation needs for n elements.
+ *   SORT_TILES      0
+ *   MERGE_RUNS      one ping-pong copy of keys (+values) and the split-point array of the
+ *                   first pass (run_len is the caller's run length)
+ *   SORT            same with run_len = BCF_TILE (run_len argument ignored)
+ *   SORT_HOST       the data itself (keys + values) plus the SORT workspace
+ *   MERGE_PAGEWISE  same as MERGE_RUNS without the split-point array
+ * Returns 0 for an invalid op / type.
+ */
+size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt);
+
+/*
+ * bcf_sort_tiles -- batched base case: ShearSort of independent 32 x 32 tiles.
+ * PAPER.md section 3.1 (L105-111), Algorithm 1 (L308-335) with the implicit transposition of
+ * section 3.3 / Algorithm 2 (L153, L337-363):  ceil(log2 w) = 5 phases of {row sort in
+ * alternating direction, column sort ascending} and one clean-up row sort, every line sorted by
+ * one thread with Batcher's odd-even mergesort in registers, every shared-memory access of a
+ * warp touching 32 distinct banks.
+ *
+ *   d_keys, d_vals : in place; tile t is elements [1024 t, 1024 t + 1024), row-major 32 x 32.
+ *   num_tiles      : number of whole tiles.
+ * On return (after the stream drains) every tile is in ascending row-major order.
+ */
+bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles,
+                          bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
+
+/*
+ * bcf_merge_partition -- split-point search of ONE merge pass (hot-path row a5).
+ * Not in the paper: it replaces the sampled bucket distribution of PAPER.md section 3.2
+ * (L131-143, Alg. 7), which the paper needs because its page-wise merge is sequential per pair
+ * (L121); north_star asks for "merge partitioning (split-point search so each CTA gets an equal
+ * share of output)".  Runs are [i*run_len, min(n,(i+1)*run_len)); runs 2p and 2p+1 form pair p
+ * (A, B).  Each pair's output is cut into shares of BCF_TILE elements; the pass has
+ *      num_shares = ceil(n / (2 run_len)) * ceil(2 run_len / BCF_TILE)
+ * share slots, slot j belonging to pair j / ceil(2 run_len / BCF_TILE).
+ *   d_splits[j] (uint32, num_shares entries, device) receives the co-rank of the share's first
+ *   output diagonal d: the number of elements of A among the first d outputs of the stable
+ *   (A-first on ties) merge of A and B, i.e. the smallest i in [max(0,d-|B|), min(d,|A|)] with
+ *   NOT (A[i] <= B[d-i-1]).  Slots past the end of a short last pair receive |A|.
+ */
+bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len,
+                               bcf_key_t kt, bcf_val_t vt, uint32_t *d_splits, size_t num_shares,
+                               bcf_stream_t stream);
+
+/*
+ * bcf_merge_runs -- BCFMergesort's merging phase on already sorted runs.
+ * PAPER.md section 3 (L103): ceil(log2(#runs)) rounds, each merging pairs of runs and each one
+ * read + one write of all n elements (Lemma 2).  Every round is one partition
+ * launch (above) and one merge launch in which a warp takes one share: it loads its piece of A
+ * and its piece of B (together BCF_TILE elements, coalesced), merges them in shared
+ * memory/registers with ONE ShearSort round -- SHEARSORT-MERGE, with the
+ * second piece stored reversed so that one {column pass, row pass} is sufficient (reading A8) --
+ * and stores BCF_TILE outputs coalesced.  Partial shares are padded with the maximum element in
+ * registers only.
+ *
+ *   d_keys_in/d_vals_in  : n elements, runs of run_len each already sorted (unchecked). Not modified.
+ *   d_keys_out/d_vals_out: receive the single sorted sequence, whatever the number of rounds.
+ *                          Must not overlap the inputs or the workspace.
+ *   d_workspace          : >= bcf_workspace_bytes(BCF_OP_MERGE_RUNS, n, run_len, kt, vt) bytes.
+ */
+bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
+                          size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
+                          void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+
+/*
+ * bcf_sort -- BCFMergesort (section 3, Appendix B): base case on
+ * ceil(n / BCF_TILE) tiles (a last partial tile is padded with the maximum element on chip
+ * only), then ceil(log2(ceil(n / BCF_TILE))) merge rounds ping-ponging between the data and the
+ * workspace.  In place: the sorted result is in d_keys / d_vals for any n.
+ *   d_workspace : >= bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt) bytes.
+ */
+bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
+                    void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+
+/*
+ * bcf_sort_host -- bcf_sort on HOST buffers (the end-to-end path bench.py's `e2e` times).
+ * Copies h_keys / h_vals (n elements, host memory, ideally pinned) to the device scratch,
+ * sorts there, copies the result back into h_keys / h_vals and SYNCHRONISES `stream` before
+ * returning, so the host buffers hold the sorted data on return.
+ *   d_scratch : >= bcf_workspace_bytes(BCF_OP_SORT_HOST, n, 0, kt, vt) bytes of device memory.
+ */
+bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
+                         void *d_scratch, size_t scratch_bytes, bcf_stream_t stream);
+
+/*
+ * bcf_merge_runs_pagewise -- the paper's own streaming form of the merge (hot-path row a7):
+ * BINARY-MERGE, Algorithm 6 (L457-490), L127, L416-420.  One warp per pair of runs
+ * keeps a page of M = BCF_TILE elements on chip, refills M/2 from the stream whose last loaded
+ * page ends smaller, merges with SHEARSORT-MERGE and emits the M/2 smallest; partial pages are
+ * padded with the maximum element on chip only.  Sequential per pair, so it only
+ * fills the GPU while there are many pairs; same arguments and result as bcf_merge_runs.
+ *   d_workspace : >= bcf_workspace_bytes(BCF_OP_MERGE_PAGEWISE, n, run_len, kt, vt) bytes.
+ */
+bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in, void *d_keys_out,
+                                   void *d_vals_out, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
+                                   void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+
+/* ------------------------------------------------------------------ measurement hooks ------ */
+
+typedef enum {
+    BCF_KERNEL_TILE_SORT = 0,
+    BCF_KERNEL_PARTITION = 1,
+    BCF_KERNEL_MERGE = 2,
+    BCF_KERNEL_MERGE_PAGEWISE = 3,
+    BCF_KERNEL_CLASSES = 4
+} bcf_kernel_class;
+
+/*
+ * Per-kernel timing with CUDA events recorded on the launching stream (bench.py's `roofline`).
+ * bcf_profile_enable(1) makes every later launch be bracketed by an event pair owned by the
+ * library (a fixed pool; when it is exhausted further launches are not timed);
+ * bcf_profile_read synchronises those events, adds up elapsed milliseconds and launch counts
+ * per kernel class into ms[BCF_KERNEL_CLASSES] / launches[BCF_KERNEL_CLASSES] (host arrays), and
+ * resets the pool.  bcf_profile_enable(0) switches timing off.  Launch COUNTS per class are kept
+ * whether or not timing is on; bcf_launch_counts copies and clears them.
+ */
+bcf_status bcf_profile_enable(int on);
+bcf_status bcf_profile_read(float *ms, unsigned long long *launches);
+void bcf_launch_counts(unsigned long long *launches);
+
+/*
+ * Static resource usage of a kernel class for an element type (needs a device):
+ * registers per thread, static+dynamic shared memory per CTA as launched, threads per CTA,
+ * resident CTAs per SM at that configuration, local-memory bytes per thread (must be 0).
+ */
+bcf_status bcf_kernel_info(int kernel_class, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread,
+                           int *smem_bytes_per_cta, int *threads_per_cta, int *ctas_per_sm,
+                           int *local_bytes_per_thread);
+
+/* ------------------------------------------------------------------ layout introspection --- */
+
+typedef enum {
+    BCF_ACCESS_ROW_STORE = 0,   /* thread r writes 16-byte chunk `step` (0..7) of logical row r      */
+    BCF_ACCESS_ROW_LOAD = 1,    /* thread r reads  16-byte chunk `step` (0..7) of logical row r      */
+    BCF_ACCESS_COL_LOAD = 2,    /* thread c reads  word `step` (0..31) of logical column c, rows of
+                                   odd index mirrored (the alternating row direction)              */
+    BCF_ACCESS_COL_STORE = 3,   /* thread c writes word `step` of logical column c (same mirroring) */
+    BCF_ACCESS_COL_STORE_PLAIN = 4, /* thread c writes word `step` of column c, no mirroring (merge) */
+    BCF_ACCESS_OUT_LOAD128 = 5, /* lane reads the 16-byte chunk it stores to global in vector store
+                                   `step` (0..7): row 4*step + lane/8, chunk lane%8               */
+    BCF_ACCESS_OUT_LOAD64 = 6,  /* lane reads 8 bytes: row 2*step + lane/16, words 2*(lane%16)..+1  */
+    BCF_ACCESS_OUT_LOAD32 = 7,  /* lane reads 1 word: row step, column lane                        */
+    BCF_ACCESS_PATTERNS = 8
+} bcf_access_pattern;
+
+/*
+ * The shared-memory word (0..1023, bank = word % 32) that holds logical element (row, col) of a
+ * 32 x 32 plane, and the words a lane touches in each access pattern the kernels use.  Pure host
+ * functions (no device needed) compiled from the SAME constexpr index functions the kernels
+ * use, so a host-side bank model can prove every warp access conflict-free
+ * (section 2.1; section 3.3).
+ *   bcf_layout_access returns the number of consecutive words (1, 2 or 4) and stores the first.
+ */
+int bcf_layout_word(int row, int col);
+int bcf_layout_access(int pattern, int step, int lane, int *first_word);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BCF_H_ */

@@ -1,0 +1,32 @@
+"""paper_1306_5076_b200 -- B200-native bank-conflict-free sorting (arXiv 1306.5076).
+
+A thin Python binding over the C-ABI CUDA library `libbcf.so` (include/bcf.h): argument
+marshalling only, every step of the path runs in the sm_100a kernels under csrc/.
+PyTorch is used for device memory and streams.  There is no CPU fallback: if the library is
+missing or the device is not a B200, calls raise.
+
+    import paper_1306_5076_b200 as bcf
+    bcf.sort_tiles(keys)                      # in place, 32x32 tiles        (bcf_sort_tiles)
+    out = bcf.merge_runs(keys, run_len)       # sorted runs -> one sequence  (bcf_merge_runs)
+    bcf.sort(keys, vals)                      # in place BCFMergesort        (bcf_sort)
+"""
+from .binding import (  # noqa: F401
+    BcfError,
+    KERNEL_CLASSES,
+    kernel_info,
+    launch_counts,
+    layout_access,
+    layout_word,
+    lib,
+    merge_partition,
+    merge_runs,
+    merge_runs_pagewise,
+    num_shares,
+    profile_enable,
+    profile_read,
+    sort,
+    sort_host,
+    sort_tiles,
+    version,
+    workspace_bytes,
+)

@@ -1,0 +1,236 @@
+"""ctypes binding of libbcf.so -- same names as the C ABI (include/bcf.h), marshalling only."""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libbcf.so")
+_LIB = None
+
+BCF_KEY_U32, BCF_KEY_U64 = 0, 1
+BCF_VAL_NONE, BCF_VAL_U32 = 0, 1
+OP_SORT_TILES, OP_MERGE_RUNS, OP_SORT, OP_SORT_HOST, OP_MERGE_PAGEWISE = range(5)
+KERNEL_CLASSES = ("tile_sort", "partition", "merge", "merge_pagewise")
+TILE = 1024
+
+
+class BcfError(RuntimeError):
+    def __init__(self, status, name, where):
+        super().__init__(f"{where}: {name} ({status})")
+        self.status = status
+        self.name = name
+
+
+def lib():
+    """Load libbcf.so (built in-tree by paper_1306_5076_b200.build).  Fails loudly if absent."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} not found: build it with `python -m paper_1306_5076_b200.build` "
+            "(there is no CPU fallback)")
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, sz, ci, u64 = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_ulonglong
+    L.bcf_status_string.restype = ctypes.c_char_p
+    L.bcf_status_string.argtypes = [ci]
+    L.bcf_version.restype = ctypes.c_char_p
+    L.bcf_workspace_bytes.restype = sz
+    L.bcf_workspace_bytes.argtypes = [ci, sz, sz, ci, ci]
+    L.bcf_sort_tiles.argtypes = [vp, vp, sz, ci, ci, vp]
+    L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_merge_runs.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_merge_runs_pagewise.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_sort.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
+    L.bcf_sort_host.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
+    L.bcf_profile_enable.argtypes = [ci]
+    L.bcf_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u64)]
+    L.bcf_launch_counts.argtypes = [ctypes.POINTER(u64)]
+    L.bcf_launch_counts.restype = None
+    L.bcf_kernel_info.argtypes = [ci, ci, ci] + [ctypes.POINTER(ci)] * 5
+    L.bcf_layout_word.argtypes = [ci, ci]
+    L.bcf_layout_access.argtypes = [ci, ci, ci, ctypes.POINTER(ci)]
+    _LIB = L
+    return L
+
+
+def _check(status, where):
+    if status != 0:
+        raise BcfError(status, lib().bcf_status_string(status).decode(), where)
+
+
+def version():
+    return lib().bcf_version().decode()
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _types(keys, vals):
+    torch = _torch()
+    if keys.dtype == torch.uint32 or keys.dtype == torch.int32:
+        kt = BCF_KEY_U32
+    elif keys.dtype == torch.uint64 or keys.dtype == torch.int64:
+        kt = BCF_KEY_U64
+    else:
+        raise TypeError(f"keys must be a 32- or 64-bit integer tensor (bit pattern = unsigned key), got {keys.dtype}")
+    if vals is None:
+        return kt, BCF_VAL_NONE
+    if vals.dtype not in (torch.uint32, torch.int32):
+        raise TypeError(f"vals must be a 32-bit integer tensor, got {vals.dtype}")
+    if vals.numel() != keys.numel():
+        raise ValueError("keys and vals must have the same number of elements")
+    return kt, BCF_VAL_U32
+
+
+def _dev(t, name):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (there is no CPU path)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def workspace_bytes(op, n, run_len=0, key_dtype=None, has_vals=False, kt=None, vt=None):
+    if kt is None:
+        torch = _torch()
+        kt = BCF_KEY_U64 if key_dtype in (torch.uint64, torch.int64, np.uint64) else BCF_KEY_U32
+    if vt is None:
+        vt = BCF_VAL_U32 if has_vals else BCF_VAL_NONE
+    return int(lib().bcf_workspace_bytes(int(op), int(n), int(run_len), kt, vt))
+
+
+def _workspace(op, n, run_len, kt, vt, device, workspace):
+    torch = _torch()
+    need = int(lib().bcf_workspace_bytes(int(op), int(n), int(run_len), kt, vt))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
+    return workspace, workspace.numel() * workspace.element_size()
+
+
+def num_shares(n, run_len):
+    """Share slots of one merge round (include/bcf.h, bcf_merge_partition)."""
+    pairs = -(-n // (2 * run_len))
+    return pairs * (-(-2 * run_len // TILE))
+
+
+def sort_tiles(keys, vals=None, stream=None):
+    """bcf_sort_tiles: in place ShearSort of consecutive 32x32 tiles."""
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    if n % TILE:
+        raise ValueError("sort_tiles needs a whole number of 1024-element tiles")
+    _check(lib().bcf_sort_tiles(_dev(keys, "keys"), _dev(vals, "vals"), n // TILE, kt, vt, _stream(stream)),
+           "bcf_sort_tiles")
+    return keys if vals is None else (keys, vals)
+
+
+def merge_partition(keys, run_len, vals=None, stream=None):
+    """bcf_merge_partition: split points (uint32 tensor) of one merge round."""
+    torch = _torch()
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    shares = num_shares(n, run_len) if n else 0
+    splits = torch.empty(max(shares, 1), dtype=torch.int32, device=keys.device)
+    _check(lib().bcf_merge_partition(_dev(keys, "keys"), _dev(vals, "vals"), n, int(run_len), kt, vt,
+                                     splits.data_ptr(), shares, _stream(stream)), "bcf_merge_partition")
+    return splits[:shares]
+
+
+def _merge(fn, name, op, keys, run_len, vals, out_keys, out_vals, workspace, stream):
+    torch = _torch()
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    if out_keys is None:
+        out_keys = torch.empty_like(keys)
+    if vals is not None and out_vals is None:
+        out_vals = torch.empty_like(vals)
+    ws, ws_bytes = _workspace(op, n, run_len, kt, vt, keys.device, workspace)
+    _check(fn(_dev(keys, "keys"), _dev(vals, "vals"), _dev(out_keys, "out_keys"), _dev(out_vals, "out_vals"),
+              n, int(run_len), kt, vt, ws.data_ptr(), ws_bytes, _stream(stream)), name)
+    return out_keys if vals is None else (out_keys, out_vals)
+
+
+def merge_runs(keys, run_len, vals=None, out_keys=None, out_vals=None, workspace=None, stream=None):
+    """bcf_merge_runs: merge sorted runs of run_len into one sorted sequence (out of place)."""
+    return _merge(lib().bcf_merge_runs, "bcf_merge_runs", OP_MERGE_RUNS, keys, run_len, vals, out_keys, out_vals,
+                  workspace, stream)
+
+
+def merge_runs_pagewise(keys, run_len, vals=None, out_keys=None, out_vals=None, workspace=None, stream=None):
+    """bcf_merge_runs_pagewise: the paper's streaming Alg. 6, one warp per pair of runs."""
+    return _merge(lib().bcf_merge_runs_pagewise, "bcf_merge_runs_pagewise", OP_MERGE_PAGEWISE, keys, run_len, vals,
+                  out_keys, out_vals, workspace, stream)
+
+
+def sort(keys, vals=None, workspace=None, stream=None):
+    """bcf_sort: in place BCFMergesort of device tensors."""
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    ws, ws_bytes = _workspace(OP_SORT, n, 0, kt, vt, keys.device, workspace)
+    _check(lib().bcf_sort(_dev(keys, "keys"), _dev(vals, "vals"), n, kt, vt, ws.data_ptr(), ws_bytes,
+                          _stream(stream)), "bcf_sort")
+    return keys if vals is None else (keys, vals)
+
+
+def sort_host(keys, vals=None, scratch=None, device="cuda", stream=None):
+    """bcf_sort_host: in place sort of HOST tensors (ideally pinned); H2D + sort + D2H + sync."""
+    torch = _torch()
+    kt, vt = _types(keys, vals)
+    if keys.is_cuda or (vals is not None and vals.is_cuda):
+        raise ValueError("sort_host takes host tensors")
+    n = keys.numel()
+    need = int(lib().bcf_workspace_bytes(OP_SORT_HOST, n, 0, kt, vt))
+    if scratch is None:
+        scratch = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
+    _check(lib().bcf_sort_host(keys.data_ptr(), None if vals is None else vals.data_ptr(), n, kt, vt,
+                               scratch.data_ptr(), scratch.numel(), _stream(stream)), "bcf_sort_host")
+    return keys if vals is None else (keys, vals)
+
+
+def profile_enable(on=True):
+    _check(lib().bcf_profile_enable(1 if on else 0), "bcf_profile_enable")
+
+
+def profile_read():
+    """{class: (milliseconds, launches)} of the launches timed since the last read."""
+    ms = (ctypes.c_float * len(KERNEL_CLASSES))()
+    cnt = (ctypes.c_ulonglong * len(KERNEL_CLASSES))()
+    _check(lib().bcf_profile_read(ms, cnt), "bcf_profile_read")
+    return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+
+def launch_counts():
+    cnt = (ctypes.c_ulonglong * len(KERNEL_CLASSES))()
+    lib().bcf_launch_counts(cnt)
+    return {k: int(cnt[i]) for i, k in enumerate(KERNEL_CLASSES)}
+
+
+def kernel_info(kernel_class, kt=BCF_KEY_U32, vt=BCF_VAL_NONE):
+    vals = [ctypes.c_int() for _ in range(5)]
+    _check(lib().bcf_kernel_info(KERNEL_CLASSES.index(kernel_class), kt, vt, *[ctypes.byref(v) for v in vals]),
+           "bcf_kernel_info")
+    names = ("regs_per_thread", "smem_bytes_per_cta", "threads_per_cta", "ctas_per_sm", "local_bytes_per_thread")
+    return dict(zip(names, (v.value for v in vals)))
+
+
+def layout_word(row, col):
+    return int(lib().bcf_layout_word(int(row), int(col)))
+
+
+def layout_access(pattern, step, lane):
+    """(first_word, words) a lane touches in one step of an access pattern (host-only)."""
+    first = ctypes.c_int()
+    nwords = lib().bcf_layout_access(int(pattern), int(step), int(lane), ctypes.byref(first))
+    return first.value, int(nwords)

@@ -1,0 +1,563 @@
+// bcf_api.cu -- the C ABI of include/bcf.h: argument validation, workspace carving, the merge-round
+// driver and the measurement hooks.  Every step of the path runs in the
+// kernels of bcf_kernels.cuh; there is no CPU fallback.
+#include "../../include/bcf.h"
+
+#include <cstdio>
+#include <cstring>
+
+#include "bcf_kernels.cuh"
+#include "bcf_pagewise.cuh"
+
+using namespace bcf;
+
+namespace {
+
+// ------------------------------------------------------------------ small host helpers
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline int ceil_log2(size_t x) { int l = 0; while ((size_t(1) << l) < x) ++l; return l; }
+inline size_t key_bytes(bcf_key_t kt) { return kt == BCF_KEY_U64 ? 8 : 4; }
+inline bool valid_types(bcf_key_t kt, bcf_val_t vt)
+{
+    return (kt == BCF_KEY_U32 || kt == BCF_KEY_U64) && (vt == BCF_VAL_NONE || vt == BCF_VAL_U32);
+}
+
+PassGeom pass_geom(size_t n, size_t run_len)
+{
+    PassGeom g;
+    g.n = n;
+    g.run_len = run_len;
+    const unsigned long long two_l = 2ull * run_len;
+    g.shares_per_pair = static_cast<unsigned int>((two_l + TILE - 1) / TILE);
+    const unsigned long long pairs = (n + two_l - 1) / two_l;
+    g.num_shares = pairs * g.shares_per_pair;
+    return g;
+}
+
+// Largest split-point array any round of merging runs of `run_len` needs.
+size_t max_shares(size_t n, size_t run_len)
+{
+    size_t m = 0;
+    for (size_t l = run_len; l < n; l *= 2) {
+        const PassGeom g = pass_geom(n, l);
+        if (g.num_shares > m) m = g.num_shares;
+    }
+    return m;
+}
+
+bcf_status check_device()
+{
+    static int cached_dev = -1;
+    static bcf_status cached = BCF_ERR_UNSUPPORTED_DEVICE;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return BCF_ERR_CUDA;
+    if (dev == cached_dev) return cached;
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return BCF_ERR_CUDA;
+    cached_dev = dev;
+    cached = (major == 10) ? BCF_OK : BCF_ERR_UNSUPPORTED_DEVICE;
+    return cached;
+}
+
+bool overlap(const void *a, size_t an, const void *b, size_t bn)
+{
+    if (!a || !b || !an || !bn) return false;
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + bn && y < x + an;
+}
+
+// ------------------------------------------------------------------ profiling (bcf_profile_*)
+
+constexpr int PROFILE_POOL = 8192;
+struct Profile {
+    bool on = false;
+    int used = 0;
+    cudaEvent_t start[PROFILE_POOL];
+    cudaEvent_t stop[PROFILE_POOL];
+    int cls[PROFILE_POOL];
+    int created = 0;
+    unsigned long long launches[BCF_KERNEL_CLASSES] = {0, 0, 0, 0};
+} g_prof;
+
+struct LaunchTimer {
+    int idx = -1;
+    cudaStream_t s;
+    LaunchTimer(int cls, cudaStream_t stream) : s(stream)
+    {
+        g_prof.launches[cls]++;
+        if (!g_prof.on || g_prof.used >= PROFILE_POOL) return;
+        idx = g_prof.used++;
+        if (idx >= g_prof.created) {
+            cudaEventCreate(&g_prof.start[idx]);
+            cudaEventCreate(&g_prof.stop[idx]);
+            g_prof.created = idx + 1;
+        }
+        g_prof.cls[idx] = cls;
+        cudaEventRecord(g_prof.start[idx], s);
+    }
+    ~LaunchTimer()
+    {
+        if (idx >= 0) cudaEventRecord(g_prof.stop[idx], s);
+    }
+};
+
+// ------------------------------------------------------------------ launchers
+
+template <class E>
+constexpr size_t warp_smem_bytes() { return size_t(E::NP) * TILE * 4; }
+
+template <class E>
+bcf_status launch_tile_sort(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n,
+                            cudaStream_t s)
+{
+    const size_t tiles = (n + TILE - 1) / TILE;
+    if (tiles == 0) return BCF_OK;
+    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(tile_sort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return BCF_ERR_CUDA;
+        attr_set = true;
+    }
+    const size_t blocks = (tiles + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
+    {
+        LaunchTimer t(BCF_KERNEL_TILE_SORT, s);
+        tile_sort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+template <class E>
+bcf_status launch_partition(const void *kin, const uint32_t *vin, uint32_t *splits, const PassGeom &g, cudaStream_t s)
+{
+    if (g.num_shares == 0) return BCF_OK;
+    const unsigned blocks = static_cast<unsigned>((g.num_shares + 127) / 128);
+    {
+        LaunchTimer t(BCF_KERNEL_PARTITION, s);
+        partition_kernel<E><<<blocks, 128, 0, s>>>(kin, vin, splits, g);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+template <class E>
+bcf_status launch_merge(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const uint32_t *splits,
+                        const PassGeom &g, cudaStream_t s)
+{
+    if (g.num_shares == 0) return BCF_OK;
+    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(merge_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return BCF_ERR_CUDA;
+        attr_set = true;
+    }
+    const unsigned blocks = static_cast<unsigned>((g.num_shares + WARPS_PER_CTA - 1) / WARPS_PER_CTA);
+    {
+        LaunchTimer t(BCF_KERNEL_MERGE, s);
+        merge_kernel<E><<<blocks, WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, splits, g);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+template <class E>
+bcf_status launch_pagewise(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, size_t run_len,
+                           cudaStream_t s)
+{
+    const size_t pairs = (n + 2 * run_len - 1) / (2 * run_len);
+    if (pairs == 0) return BCF_OK;
+    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(pagewise_merge_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return BCF_ERR_CUDA;
+        attr_set = true;
+    }
+    const unsigned blocks = static_cast<unsigned>((pairs + WARPS_PER_CTA - 1) / WARPS_PER_CTA);
+    {
+        LaunchTimer t(BCF_KERNEL_MERGE_PAGEWISE, s);
+        pagewise_merge_kernel<E><<<blocks, WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n, run_len);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+// Dispatch a templated callable on the runtime element type.
+#define BCF_DISPATCH(kt, vt, CALL)                                                   \
+    do {                                                                             \
+        if ((kt) == BCF_KEY_U32 && (vt) == BCF_VAL_NONE) { using E = Elem<1, false>; CALL; } \
+        else if ((kt) == BCF_KEY_U32) { using E = Elem<1, true>; CALL; }             \
+        else if ((vt) == BCF_VAL_NONE) { using E = Elem<2, false>; CALL; }           \
+        else { using E = Elem<2, true>; CALL; }                                      \
+    } while (0)
+
+struct Workspace {
+    void *keys;
+    uint32_t *vals;
+    uint32_t *splits;
+    size_t bytes;
+};
+
+// Carve [keys copy][vals copy][splits] out of a workspace; any of the three can be empty.
+Workspace carve(void *base, size_t n, bcf_key_t kt, bcf_val_t vt, bool with_data, size_t shares)
+{
+    Workspace w;
+    size_t off = 0;
+    char *b = static_cast<char *>(base);
+    w.keys = b ? b + off : nullptr;
+    if (with_data) off += align_up(n * key_bytes(kt), 256);
+    w.vals = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
+    if (with_data && vt == BCF_VAL_U32) off += align_up(n * 4, 256);
+    w.splits = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
+    off += align_up((shares + 1) * 4, 256);
+    w.bytes = off;
+    return w;
+}
+
+// The merging phase: `rounds` rounds starting from sorted runs of run_len in
+// (k0, v0); round r writes to dst[r].  Each round = partition + merge, one read + one write of
+// all n elements (Lemma 2).
+template <class E>
+bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
+                        bool first_to_a, size_t n, size_t run_len, uint32_t *splits, cudaStream_t s)
+{
+    const void *ksrc = k0;
+    const uint32_t *vsrc = v0;
+    bool to_a = first_to_a;
+    for (size_t l = run_len; l < n; l *= 2) {
+        const PassGeom g = pass_geom(n, l);
+        void *kd = to_a ? ka : kb;
+        uint32_t *vd = to_a ? va : vb;
+        bcf_status st = launch_partition<E>(ksrc, vsrc, splits, g, s);
+        if (st != BCF_OK) return st;
+        st = launch_merge<E>(ksrc, vsrc, kd, vd, splits, g, s);
+        if (st != BCF_OK) return st;
+        ksrc = kd;
+        vsrc = vd;
+        to_a = !to_a;
+    }
+    return BCF_OK;
+}
+
+template <class E>
+bcf_status pagewise_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
+                           bool first_to_a, size_t n, size_t run_len, cudaStream_t s)
+{
+    const void *ksrc = k0;
+    const uint32_t *vsrc = v0;
+    bool to_a = first_to_a;
+    for (size_t l = run_len; l < n; l *= 2) {
+        void *kd = to_a ? ka : kb;
+        uint32_t *vd = to_a ? va : vb;
+        bcf_status st = launch_pagewise<E>(ksrc, vsrc, kd, vd, n, l, s);
+        if (st != BCF_OK) return st;
+        ksrc = kd;
+        vsrc = vd;
+        to_a = !to_a;
+    }
+    return BCF_OK;
+}
+
+bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d_vals_in, void *d_keys_out,
+                             void *d_vals_out, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
+                             void *d_workspace, size_t workspace_bytes, cudaStream_t s)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_keys_out) return BCF_ERR_INVALID_ARG;
+    if ((vt == BCF_VAL_U32) != (d_vals_in != nullptr) || (vt == BCF_VAL_U32) != (d_vals_out != nullptr))
+        return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_vals_in) || !aligned16(d_vals_out) ||
+        !aligned16(d_workspace))
+        return BCF_ERR_MISALIGNED;
+    const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
+    if (overlap(d_keys_in, kb, d_keys_out, kb) || overlap(d_vals_in, vb, d_vals_out, vb) ||
+        overlap(d_keys_in, kb, d_vals_out, vb) || overlap(d_vals_in, vb, d_keys_out, kb))
+        return BCF_ERR_INVALID_ARG;
+    const size_t need = bcf_workspace_bytes(pagewise ? BCF_OP_MERGE_PAGEWISE : BCF_OP_MERGE_RUNS, n, run_len, kt, vt);
+    if (need && (!d_workspace || workspace_bytes < need)) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    if (overlap(d_workspace, need, d_keys_in, kb) || overlap(d_workspace, need, d_keys_out, kb) ||
+        overlap(d_workspace, need, d_vals_in, vb) || overlap(d_workspace, need, d_vals_out, vb))
+        return BCF_ERR_INVALID_ARG;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+
+    const size_t runs = (n + run_len - 1) / run_len;
+    const int rounds = ceil_log2(runs);
+    if (rounds == 0) {   // a single run: the result is the input
+        if (cudaMemcpyAsync(d_keys_out, d_keys_in, kb, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BCF_ERR_CUDA;
+        if (vb && cudaMemcpyAsync(d_vals_out, d_vals_in, vb, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BCF_ERR_CUDA;
+        return BCF_OK;
+    }
+    const Workspace w = carve(d_workspace, n, kt, vt, rounds >= 2, pagewise ? 0 : max_shares(n, run_len));
+    // round r (1-based) writes to `out` when (rounds - r) is even, so the last round lands in out.
+    const bool first_to_out = ((rounds - 1) % 2 == 0);
+    if (pagewise) {
+        BCF_DISPATCH(kt, vt, st = pagewise_rounds<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
+                                                     static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out,
+                                                     n, run_len, s));
+    } else {
+        BCF_DISPATCH(kt, vt, st = merge_rounds<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
+                                                  static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out, n,
+                                                  run_len, w.splits, s));
+    }
+    return st;
+}
+
+}  // namespace
+
+// ====================================================================== exported C ABI
+
+extern "C" {
+
+const char *bcf_status_string(bcf_status s)
+{
+    switch (s) {
+    case BCF_OK: return "BCF_OK";
+    case BCF_ERR_INVALID_ARG: return "BCF_ERR_INVALID_ARG";
+    case BCF_ERR_MISALIGNED: return "BCF_ERR_MISALIGNED";
+    case BCF_ERR_WORKSPACE_TOO_SMALL: return "BCF_ERR_WORKSPACE_TOO_SMALL";
+    case BCF_ERR_UNSUPPORTED_DEVICE: return "BCF_ERR_UNSUPPORTED_DEVICE";
+    case BCF_ERR_CUDA: return "BCF_ERR_CUDA";
+    }
+    return "BCF_ERR_UNKNOWN";
+}
+
+const char *bcf_version(void) { return "bcf 0.1 (sm_100a)"; }
+
+size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
+{
+    if (!valid_types(kt, vt) || n == 0) return 0;
+    switch (op) {
+    case BCF_OP_SORT_TILES:
+        return 0;
+    case BCF_OP_MERGE_RUNS: {
+        if (run_len == 0) return 0;
+        const int rounds = ceil_log2((n + run_len - 1) / run_len);
+        if (rounds == 0) return 0;
+        return carve(nullptr, n, kt, vt, rounds >= 2, max_shares(n, run_len)).bytes;
+    }
+    case BCF_OP_MERGE_PAGEWISE: {
+        if (run_len == 0) return 0;
+        const int rounds = ceil_log2((n + run_len - 1) / run_len);
+        if (rounds < 2) return 0;
+        return carve(nullptr, n, kt, vt, true, 0).bytes;
+    }
+    case BCF_OP_SORT:
+        if (n <= TILE) return 0;
+        return carve(nullptr, n, kt, vt, true, max_shares(n, TILE)).bytes;
+    case BCF_OP_SORT_HOST: {
+        size_t data = align_up(n * key_bytes(kt), 256) + (vt == BCF_VAL_U32 ? align_up(n * 4, 256) : 0);
+        return data + bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt);
+    }
+    }
+    return 0;
+}
+
+bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (num_tiles == 0) return BCF_OK;
+    if (num_tiles >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys) || !aligned16(d_vals)) return BCF_ERR_MISALIGNED;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, static_cast<uint32_t *>(d_vals), d_keys,
+                                                  static_cast<uint32_t *>(d_vals), num_tiles * TILE, stream));
+    return st;
+}
+
+bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
+                               bcf_val_t vt, uint32_t *d_splits, size_t num_shares, bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_splits || (vt == BCF_VAL_U32) != (d_vals_in != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_vals_in)) return BCF_ERR_MISALIGNED;
+    const PassGeom g = pass_geom(n, run_len);
+    if (num_shares != g.num_shares) return BCF_ERR_INVALID_ARG;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    BCF_DISPATCH(kt, vt, st = launch_partition<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, g, stream));
+    return st;
+}
+
+bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out, size_t n,
+                          size_t run_len, bcf_key_t kt, bcf_val_t vt, void *d_workspace, size_t workspace_bytes,
+                          bcf_stream_t stream)
+{
+    return merge_runs_common(false, d_keys_in, d_vals_in, d_keys_out, d_vals_out, n, run_len, kt, vt, d_workspace,
+                             workspace_bytes, stream);
+}
+
+bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
+                                   size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt, void *d_workspace,
+                                   size_t workspace_bytes, bcf_stream_t stream)
+{
+    return merge_runs_common(true, d_keys_in, d_vals_in, d_keys_out, d_vals_out, n, run_len, kt, vt, d_workspace,
+                             workspace_bytes, stream);
+}
+
+bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_workspace,
+                    size_t workspace_bytes, bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys) || !aligned16(d_vals) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    const size_t need = bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt);
+    if (need && (!d_workspace || workspace_bytes < need)) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
+    if (overlap(d_workspace, need, d_keys, kb) || overlap(d_workspace, need, d_vals, vb)) return BCF_ERR_INVALID_ARG;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+
+    const size_t tiles = (n + TILE - 1) / TILE;
+    const int rounds = ceil_log2(tiles);
+    const Workspace w = carve(d_workspace, n, kt, vt, rounds > 0, rounds > 0 ? max_shares(n, TILE) : 0);
+    uint32_t *vals = static_cast<uint32_t *>(d_vals);
+    // With an odd number of merge rounds the base case writes into the workspace, so that the
+    // last round lands in the caller's buffer without an extra copy.
+    const bool base_to_ws = (rounds % 2 == 1);
+    void *k0 = base_to_ws ? w.keys : d_keys;
+    uint32_t *v0 = base_to_ws ? w.vals : vals;
+    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream));
+    if (st != BCF_OK || rounds == 0) return st;
+    // round 1 writes to the buffer the base case did not write.
+    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, TILE,
+                                              w.splits, stream));
+    return st;
+}
+
+bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_scratch,
+                         size_t scratch_bytes, bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32)) return BCF_ERR_INVALID_ARG;
+    if (!h_keys || (vt == BCF_VAL_U32) != (h_vals != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_scratch)) return BCF_ERR_MISALIGNED;
+    const size_t need = bcf_workspace_bytes(BCF_OP_SORT_HOST, n, 0, kt, vt);
+    if (!d_scratch || scratch_bytes < need) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
+    char *base = static_cast<char *>(d_scratch);
+    void *dk = base;
+    void *dv = vb ? base + align_up(kb, 256) : nullptr;
+    const size_t data = align_up(kb, 256) + (vb ? align_up(vb, 256) : 0);
+    if (cudaMemcpyAsync(dk, h_keys, kb, cudaMemcpyHostToDevice, stream) != cudaSuccess) return BCF_ERR_CUDA;
+    if (vb && cudaMemcpyAsync(dv, h_vals, vb, cudaMemcpyHostToDevice, stream) != cudaSuccess) return BCF_ERR_CUDA;
+    const bcf_status st = bcf_sort(dk, dv, n, kt, vt, base + data, scratch_bytes - data, stream);
+    if (st != BCF_OK) return st;
+    if (cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream) != cudaSuccess) return BCF_ERR_CUDA;
+    if (vb && cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream) != cudaSuccess) return BCF_ERR_CUDA;
+    if (cudaStreamSynchronize(stream) != cudaSuccess) return BCF_ERR_CUDA;
+    return BCF_OK;
+}
+
+// ------------------------------------------------------------------ measurement hooks
+
+bcf_status bcf_profile_enable(int on)
+{
+    g_prof.on = on != 0;
+    g_prof.used = 0;
+    return BCF_OK;
+}
+
+bcf_status bcf_profile_read(float *ms, unsigned long long *launches)
+{
+    if (!ms || !launches) return BCF_ERR_INVALID_ARG;
+    for (int c = 0; c < BCF_KERNEL_CLASSES; ++c) { ms[c] = 0.f; launches[c] = 0; }
+    for (int i = 0; i < g_prof.used; ++i) {
+        if (cudaEventSynchronize(g_prof.stop[i]) != cudaSuccess) return BCF_ERR_CUDA;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, g_prof.start[i], g_prof.stop[i]) != cudaSuccess) return BCF_ERR_CUDA;
+        ms[g_prof.cls[i]] += t;
+        launches[g_prof.cls[i]]++;
+    }
+    g_prof.used = 0;
+    return BCF_OK;
+}
+
+void bcf_launch_counts(unsigned long long *launches)
+{
+    for (int c = 0; c < BCF_KERNEL_CLASSES; ++c) {
+        if (launches) launches[c] = g_prof.launches[c];
+        g_prof.launches[c] = 0;
+    }
+}
+
+bcf_status bcf_kernel_info(int kernel_class, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread, int *smem_bytes_per_cta,
+                           int *threads_per_cta, int *ctas_per_sm, int *local_bytes_per_thread)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    const void *fn = nullptr;
+    size_t smem = 0;
+    int threads = WARPS_PER_CTA * 32;
+    BCF_DISPATCH(kt, vt, {
+        switch (kernel_class) {
+        case BCF_KERNEL_TILE_SORT: fn = (const void *)tile_sort_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
+        case BCF_KERNEL_PARTITION: fn = (const void *)partition_kernel<E>; smem = 0; threads = 128; break;
+        case BCF_KERNEL_MERGE: fn = (const void *)merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
+        case BCF_KERNEL_MERGE_PAGEWISE: fn = (const void *)pagewise_merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
+        default: break;
+        }
+    });
+    if (!fn) return BCF_ERR_INVALID_ARG;
+    cudaFuncAttributes a;
+    if (cudaFuncGetAttributes(&a, fn) != cudaSuccess) return BCF_ERR_CUDA;
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return BCF_ERR_CUDA;
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem) != cudaSuccess) return BCF_ERR_CUDA;
+    if (regs_per_thread) *regs_per_thread = a.numRegs;
+    if (smem_bytes_per_cta) *smem_bytes_per_cta = static_cast<int>(a.sharedSizeBytes + smem);
+    if (threads_per_cta) *threads_per_cta = threads;
+    if (ctas_per_sm) *ctas_per_sm = occ;
+    if (local_bytes_per_thread) *local_bytes_per_thread = static_cast<int>(a.localSizeBytes);
+    return BCF_OK;
+}
+
+// ------------------------------------------------------------------ layout introspection (host only)
+
+int bcf_layout_word(int row, int col)
+{
+    if (row < 0 || row > 31 || col < 0 || col > 31) return -1;
+    return elem_word(row, col);
+}
+
+int bcf_layout_access(int pattern, int step, int lane, int *first_word)
+{
+    if (!first_word || lane < 0 || lane > 31 || step < 0) return 0;
+    switch (pattern) {
+    case BCF_ACCESS_ROW_STORE:
+    case BCF_ACCESS_ROW_LOAD:
+        if (step > 7) return 0;
+        *first_word = chunk_word(lane, step);
+        return 4;
+    case BCF_ACCESS_COL_LOAD:
+    case BCF_ACCESS_COL_STORE:
+        if (step > 31) return 0;
+        *first_word = elem_word(step, mirrored_col(step, lane));
+        return 1;
+    case BCF_ACCESS_COL_STORE_PLAIN:
+    case BCF_ACCESS_OUT_LOAD32:
+        if (step > 31) return 0;
+        *first_word = elem_word(step, lane);
+        return 1;
+    case BCF_ACCESS_OUT_LOAD128:
+        if (step > 7) return 0;
+        *first_word = chunk_word(4 * step + (lane >> 3), lane & 7);
+        return 4;
+    case BCF_ACCESS_OUT_LOAD64:
+        if (step > 15) return 0;
+        *first_word = elem_word(2 * step + (lane >> 4), 2 * (lane & 15));
+        return 2;
+    }
+    return 0;
+}
+
+}  // extern "C"

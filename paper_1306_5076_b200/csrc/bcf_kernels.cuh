@@ -1,0 +1,337 @@
+// bcf_kernels.cuh -- the sm_100a kernels of the hot path.
+//
+//   tile_sort_kernel   a1-a4, a9 : ShearSort of 32 x 32 tiles, one warp per tile
+//   partition_kernel   a5        : split-point (co-rank) search, one thread per output share
+//   merge_kernel       a6, a8, a9: one warp per share of 1024 outputs, SHEARSORT-MERGE in registers
+//
+// One warp works alone on one tile/share: its 32 threads are the paper's "w threads" and own the
+// 32 lines of the tile ("each thread processes a separate row of the matrix").
+// Warps never talk to each other, so the only barrier in these kernels is __syncwarp(), which
+// replaces the implicit lock-step the paper relies on and is required on every
+// architecture since sm_70.
+#pragma once
+#include "bcf_core.cuh"
+
+namespace bcf {
+
+constexpr int WARPS_PER_CTA = 4;
+constexpr uint32_t SENTINEL = 0xFFFFFFFFu;   // "infinity" in every plane (reading A10)
+
+// ------------------------------------------------------------------ global memory access
+
+// Element `g` of the SoA arrays into planes of register slot k.
+template <class E>
+__device__ __forceinline__ void load_elem(const void *keys, const uint32_t *vals, const size_t g,
+                                          uint32_t (&v)[E::NP][32], const int k)
+{
+    if constexpr (E::KEY_WORDS == 1) {
+        v[0][k] = static_cast<const uint32_t *>(keys)[g];
+    } else {
+        const uint2 t = reinterpret_cast<const uint2 *>(keys)[g];
+        v[0][k] = t.y;   // high word first: planes are compared in order
+        v[1][k] = t.x;
+    }
+    if constexpr (E::HAS_VAL) v[E::KEY_WORDS][k] = vals[g];
+}
+
+template <class E>
+__device__ __forceinline__ void set_sentinel(uint32_t (&v)[E::NP][32], const int k)
+{
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) v[p][k] = SENTINEL;
+}
+
+// A1: whole tile, 128-bit coalesced loads.  Which 32 elements a thread receives is irrelevant:
+// the first step of ShearSort is a full sort of each row and the sorted tile is unique, so every
+// assignment of the tile's elements to rows gives the same result.
+template <class E>
+__device__ __forceinline__ void load_tile_vec(const void *keys, const uint32_t *vals, const size_t base,
+                                              const int lane, uint32_t (&v)[E::NP][32])
+{
+    if constexpr (E::KEY_WORDS == 1) {
+        const uint4 *pk = reinterpret_cast<const uint4 *>(static_cast<const uint32_t *>(keys) + base);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const uint4 t = pk[32 * m + lane];
+            v[0][4 * m] = t.x; v[0][4 * m + 1] = t.y; v[0][4 * m + 2] = t.z; v[0][4 * m + 3] = t.w;
+        }
+        if constexpr (E::HAS_VAL) {
+            const uint4 *pv = reinterpret_cast<const uint4 *>(vals + base);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const uint4 t = pv[32 * m + lane];
+                v[1][4 * m] = t.x; v[1][4 * m + 1] = t.y; v[1][4 * m + 2] = t.z; v[1][4 * m + 3] = t.w;
+            }
+        }
+    } else {
+        const uint4 *pk = reinterpret_cast<const uint4 *>(static_cast<const uint64_t *>(keys) + base);
+#pragma unroll
+        for (int m = 0; m < 16; ++m) {
+            const uint4 t = pk[32 * m + lane];   // keys 64m + 2 lane, +1
+            v[0][2 * m] = t.y; v[1][2 * m] = t.x; v[0][2 * m + 1] = t.w; v[1][2 * m + 1] = t.z;
+        }
+        if constexpr (E::HAS_VAL) {
+            const uint2 *pv = reinterpret_cast<const uint2 *>(vals + base);
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {
+                const uint2 t = pv[32 * m + lane];
+                v[2][2 * m] = t.x; v[2][2 * m + 1] = t.y;
+            }
+        }
+    }
+}
+
+// Partial tile (a9): element 32k + lane, padded with the sentinel past `cnt`.
+template <class E>
+__device__ __forceinline__ void load_tile_guarded(const void *keys, const uint32_t *vals, const size_t base,
+                                                  const int cnt, const int lane, uint32_t (&v)[E::NP][32])
+{
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        if (32 * k + lane < cnt) load_elem<E>(keys, vals, base + 32 * k + lane, v, k);
+        else set_sentinel<E>(v, k);
+    }
+}
+
+// A4: thread r holds sorted logical row r.  Stage through the skewed planes (row_store), then
+// every lane reads back the chunk it stores to global so that the global stores are coalesced
+// 128-bit (or 64-bit) vector stores; the reads are conflict-free (bcf_layout.cuh).  This is the
+// un-skew step of PAPER.md Alg. 2 L361-362 folded into the read pattern of the final store
+// (reading A6: the step as printed has a 2-way conflict).
+// `vec_ok`: the share is full and its global start is 16-byte aligned.
+template <class E>
+__device__ __forceinline__ void store_rows(uint32_t *planes, void *keys, uint32_t *vals, const size_t base,
+                                           const int cnt, const bool vec_ok, const int lane,
+                                           const uint32_t (&v)[E::NP][32])
+{
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) row_store(planes + p * TILE, v[p], lane);
+    __syncwarp();
+    if (vec_ok) {
+        if constexpr (E::KEY_WORDS == 1) {
+            uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint32_t *>(keys) + base);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
+                pk[32 * m + lane] = *reinterpret_cast<const uint4 *>(planes + w);
+            }
+            if constexpr (E::HAS_VAL) {
+                uint4 *pv = reinterpret_cast<uint4 *>(vals + base);
+#pragma unroll
+                for (int m = 0; m < 8; ++m) {
+                    const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
+                    pv[32 * m + lane] = *reinterpret_cast<const uint4 *>(planes + TILE + w);
+                }
+            }
+        } else {
+            uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint64_t *>(keys) + base);
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {
+                const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
+                const uint2 hi = *reinterpret_cast<const uint2 *>(planes + w);
+                const uint2 lo = *reinterpret_cast<const uint2 *>(planes + TILE + w);
+                pk[32 * m + lane] = make_uint4(lo.x, hi.x, lo.y, hi.y);
+            }
+            if constexpr (E::HAS_VAL) {
+                uint2 *pv = reinterpret_cast<uint2 *>(vals + base);
+#pragma unroll
+                for (int m = 0; m < 16; ++m) {
+                    const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
+                    pv[32 * m + lane] = *reinterpret_cast<const uint2 *>(planes + 2 * TILE + w);
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if (32 * k + lane < cnt) {
+                const int w = elem_word(k, lane);
+                const size_t g = base + 32 * k + lane;
+                if constexpr (E::KEY_WORDS == 1) {
+                    static_cast<uint32_t *>(keys)[g] = planes[w];
+                } else {
+                    reinterpret_cast<uint2 *>(keys)[g] = make_uint2(planes[TILE + w], planes[w]);
+                }
+                if constexpr (E::HAS_VAL) vals[g] = planes[E::KEY_WORDS * TILE + w];
+            }
+        }
+    }
+    __syncwarp();   // the planes are reused by the warp's next tile
+}
+
+// ------------------------------------------------------------------ a1-a4: tile ShearSort
+//
+// PAPER.md Alg. 1 (L308-335) with the transposes removed as in section 3.3 / Alg. 2:
+//   FOR i IN 1..log2(w):  row sort (alternating)   -> thread r sorts logical row r in registers
+//                         column sort (ascending)  -> thread c sorts logical column c
+//   clean-up row sort (ascending), store.
+// Row data moves registers -> planes with 8 STS.128, planes -> column registers with 32 LDS.32
+// (odd rows mirrored = descending rows), back with 32 STS.32 and 8 LDS.128; every one of these
+// warp accesses hits 32 distinct banks.
+template <class E>
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32)
+tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint32_t *planes = smem + warp * (E::NP * TILE);
+    const size_t num_tiles = (n + TILE - 1) / TILE;
+    const size_t stride = static_cast<size_t>(gridDim.x) * WARPS_PER_CTA;
+
+    for (size_t tile = static_cast<size_t>(blockIdx.x) * WARPS_PER_CTA + warp; tile < num_tiles; tile += stride) {
+        const size_t base = tile * TILE;
+        const int cnt = (n - base) < static_cast<size_t>(TILE) ? static_cast<int>(n - base) : TILE;
+        uint32_t v[E::NP][32];
+        if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
+        else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);
+
+#pragma unroll 1
+        for (int phase = 0; phase < 5; ++phase) {          // ceil(log2 32) phases (reading A2)
+            line_sort<E::NP>(v);                            // rows (ascending in registers)
+#pragma unroll
+            for (int p = 0; p < E::NP; ++p) row_store(planes + p * TILE, v[p], lane);
+            __syncwarp();
+#pragma unroll
+            for (int p = 0; p < E::NP; ++p) col_load<true>(planes + p * TILE, v[p], lane);
+            line_sort<E::NP>(v);                            // columns, ascending
+#pragma unroll
+            for (int p = 0; p < E::NP; ++p) col_store<true>(planes + p * TILE, v[p], lane);
+            __syncwarp();
+#pragma unroll
+            for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
+        }
+        line_sort<E::NP>(v);                                // clean-up pass: all rows ascending
+        store_rows<E>(planes, kout, vout, base, cnt, cnt == TILE, lane, v);
+    }
+}
+
+// ------------------------------------------------------------------ a5: merge partitioning
+
+struct PassGeom {
+    unsigned long long n;         // elements
+    unsigned long long run_len;   // L
+    unsigned int shares_per_pair; // ceil(2L / 1024)
+    unsigned long long num_shares;
+};
+
+template <class E>
+__device__ __forceinline__ bool elem_le_global(const void *keys, const uint32_t *vals, const size_t ia, const size_t ib)
+{
+    if constexpr (E::KEY_WORDS == 1) {
+        const uint32_t ka = __ldg(static_cast<const uint32_t *>(keys) + ia);
+        const uint32_t kb = __ldg(static_cast<const uint32_t *>(keys) + ib);
+        if constexpr (E::HAS_VAL) {
+            if (ka != kb) return ka < kb;
+            return __ldg(vals + ia) <= __ldg(vals + ib);
+        } else {
+            return ka <= kb;
+        }
+    } else {
+        const unsigned long long ka = __ldg(static_cast<const unsigned long long *>(keys) + ia);
+        const unsigned long long kb = __ldg(static_cast<const unsigned long long *>(keys) + ib);
+        if constexpr (E::HAS_VAL) {
+            if (ka != kb) return ka < kb;
+            return __ldg(vals + ia) <= __ldg(vals + ib);
+        } else {
+            return ka <= kb;
+        }
+    }
+}
+
+// One thread per share slot: binary search on the share's first output diagonal for the unique
+// split (i, d - i) with A[i-1] <= B[d-i] and B[d-i-1] < A[i] (A-first ties, include/bcf.h).
+template <class E>
+__global__ void __launch_bounds__(128)
+partition_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
+                 uint32_t *__restrict__ splits, const PassGeom g)
+{
+    const unsigned long long slot = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (slot >= g.num_shares) return;
+    const unsigned long long pair = slot / g.shares_per_pair;
+    const unsigned long long t = slot % g.shares_per_pair;
+    const unsigned long long a0 = pair * 2ull * g.run_len;
+    if (a0 >= g.n) { splits[slot] = 0; return; }
+    const unsigned long long alen = min(g.run_len, g.n - a0);
+    const unsigned long long b0 = a0 + alen;
+    const unsigned long long blen = min(g.run_len, g.n - b0);
+    const unsigned long long d = min(t * TILE, alen + blen);
+    unsigned long long lo = d > blen ? d - blen : 0ull;
+    unsigned long long hi = min(d, alen);
+    while (lo < hi) {
+        const unsigned long long mid = (lo + hi) >> 1;
+        if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
+        else hi = mid;
+    }
+    splits[slot] = static_cast<uint32_t>(lo);
+}
+
+// ------------------------------------------------------------------ a6: conflict-free in-smem merge
+//
+// SHEARSORT-MERGE of one share: the warp's piece of A ascending followed by
+// its piece of B REVERSED forms a bitonic sequence S of 1024 elements (padding, if any, sits in
+// the middle as the maximum), seen as a row-major 32 x 32 page.  One ShearSort round, columns
+// first: each column of S is bitonic, so the column "sort" is a 5-stage merger in the registers of
+// thread c; afterwards every row is bitonic and all elements of row r are <= those of row r+1, so
+// the row "sort" is a second 5-stage merger in the registers of thread r (reading A8).
+//  * position 32k + lane is what a coalesced global load hands to lane `lane` in its k-th load:
+//    the column layout comes straight from global memory, no shared-memory traffic;
+//  * columns -> rows through the skewed planes: 32 STS.32 + 8 LDS.128 per plane, conflict-free;
+//  * rows -> global through store_rows: 8 STS.128 + 8 LDS.128 + 8 STG.128 per plane.
+template <class E>
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32)
+merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
+             void *__restrict__ kout, uint32_t *__restrict__ vout,
+             const uint32_t *__restrict__ splits, const PassGeom g)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint32_t *planes = smem + warp * (E::NP * TILE);
+    const unsigned long long stride = static_cast<unsigned long long>(gridDim.x) * WARPS_PER_CTA;
+
+    for (unsigned long long slot = static_cast<unsigned long long>(blockIdx.x) * WARPS_PER_CTA + warp;
+         slot < g.num_shares; slot += stride) {
+        const unsigned long long pair = slot / g.shares_per_pair;
+        const unsigned int t = static_cast<unsigned int>(slot % g.shares_per_pair);
+        const unsigned long long a0 = pair * 2ull * g.run_len;
+        if (a0 >= g.n) continue;
+        const unsigned long long alen = min(g.run_len, g.n - a0);
+        const unsigned long long b0 = a0 + alen;
+        const unsigned long long blen = min(g.run_len, g.n - b0);
+        const unsigned long long plen = alen + blen;
+        const unsigned long long d0 = static_cast<unsigned long long>(t) * TILE;
+        if (d0 >= plen) continue;
+        const unsigned long long d1 = min(d0 + TILE, plen);
+        const unsigned long long i0 = splits[slot];
+        const unsigned long long i1 = (t + 1 < g.shares_per_pair) ? splits[slot + 1] : alen;
+        const int a = static_cast<int>(i1 - i0);                 // elements taken from A
+        const int b = static_cast<int>((d1 - i1) - (d0 - i0));   // elements taken from B
+        const size_t ga = a0 + i0;                               // first element of the A piece
+        const size_t gb = b0 + (d0 - i0);                        // first element of the B piece
+
+        uint32_t v[E::NP][32];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            const int p = 32 * k + lane;
+            if (p < a) load_elem<E>(kin, vin, ga + p, v, k);
+            else if (p >= TILE - b) load_elem<E>(kin, vin, gb + (TILE - 1 - p), v, k);
+            else set_sentinel<E>(v, k);
+        }
+        line_bitonic_merge<E::NP>(v);                            // column pass (strides 512..32)
+#pragma unroll
+        for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
+        __syncwarp();
+#pragma unroll
+        for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
+        line_bitonic_merge<E::NP>(v);                            // row pass (strides 16..1)
+
+        const size_t out = a0 + d0;
+        const int cnt = static_cast<int>(d1 - d0);
+        const bool vec_ok = (cnt == TILE) && ((out * E::KEY_BYTES) % 16 == 0) &&
+                            (!E::HAS_VAL || (out * 4) % 16 == 0);
+        store_rows<E>(planes, kout, vout, out, cnt, vec_ok, lane, v);
+    }
+}
+
+}  // namespace bcf

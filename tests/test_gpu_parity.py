@@ -1,0 +1,261 @@
+"""GPU parity: the CUDA path through the C ABI (paper_1306_5076_b200 -> libbcf.so) against the CPU
+oracle, element by element, bit-exact (integer work), on the same seeded inputs.  Sizes span several
+tiles/shares and ragged tails; every element type; the degenerate cases of the method."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1306_5076_b200 import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bcf():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1306_5076_b200 as m
+    m.lib()  # fail loudly if the extension is missing
+    return m
+
+
+def dev(a):
+    """numpy unsigned array -> CUDA tensor holding the same bit pattern."""
+    if a is None:
+        return None
+    signed = {np.dtype(np.uint32): np.int32, np.dtype(np.uint64): np.int64}[a.dtype]
+    return torch.from_numpy(np.ascontiguousarray(a).view(signed)).cuda()
+
+
+def host(t, like):
+    return t.cpu().numpy().view(like.dtype)
+
+
+def make(kind, n, seed, dup=False):
+    """(keys, vals) numpy arrays of element type `kind` in {'u32','u32u32','u64','u64u32'}."""
+    rng = np.random.default_rng(seed)
+    hi = 16 if dup else (1 << 32)
+    if kind.startswith("u32"):
+        keys = rng.integers(0, hi, size=n, dtype=np.uint64).astype(np.uint32)
+    else:
+        keys = rng.integers(0, hi, size=n, dtype=np.uint64)
+        if not dup:
+            keys = (keys << np.uint64(32)) | rng.integers(0, 1 << 32, size=n, dtype=np.uint64)
+            keys[::7] &= np.uint64(0xFFFFFFFF)          # equal high words, order decided by the low word
+    vals = None
+    if kind.endswith("u32") and kind not in ("u32",):
+        vals = rng.permutation(n).astype(np.uint32) if n else np.zeros(0, np.uint32)
+    if n > 8:                                            # the padding value is a legal element (A10)
+        keys[n // 3] = np.iinfo(keys.dtype).max
+        if vals is not None:
+            vals[n // 3] = 0xFFFFFFFF
+    return keys, vals
+
+
+KINDS = ["u32", "u32u32", "u64", "u64u32"]
+
+
+def assert_same(got_k, got_v, want, vals):
+    if vals is None:
+        assert np.array_equal(got_k, want)
+    else:
+        assert np.array_equal(got_k, want[0])
+        assert np.array_equal(got_v, want[1])
+
+
+# ---------------------------------------------------------------- bcf_sort_tiles (a1-a4)
+
+
+def test_sort_tiles_config1_exact(bcf):
+    """BASELINE config 1 at full size: 1024 tiles of uint32, uniform."""
+    keys = workloads.cfg1_tiles_u32()
+    d = dev(keys)
+    bcf.sort_tiles(d)
+    assert np.array_equal(host(d, keys), oracle.shearsort_tiles(keys))
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("tiles", [1, 3, 4, 9, 130])
+def test_sort_tiles_types_and_counts(bcf, kind, tiles):
+    keys, vals = make(kind, tiles * 1024, seed=tiles, dup=(tiles == 9))
+    if tiles >= 3:
+        keys[1024:2048] = keys[1024]                                    # all-equal tile
+        keys[2048:3072] = np.sort(keys[2048:3072])[::-1]                # reversed tile
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort_tiles(dk, dv)
+    want = oracle.shearsort_tiles(keys, vals)
+    assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+def test_sort_tiles_config2_shape(bcf):
+    """Config 2 recipe (keys in [0,16), value = index) on 256 tiles; equals a stable sort by key."""
+    keys, vals = workloads.cfg2_tiles_u32_u32(num_tiles=256)
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort_tiles(dk, dv)
+    wk, wv = oracle.shearsort_tiles(keys, vals)
+    assert np.array_equal(host(dk, keys), wk) and np.array_equal(host(dv, vals), wv)
+
+
+# ---------------------------------------------------------------- bcf_merge_partition (a5)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("n,run_len", [(5000, 1024), (8192, 4096), (3000, 700), (4096, 2048), (2500, 3000)])
+def test_merge_partition_matches_oracle_corank(bcf, kind, n, run_len):
+    keys, vals = make(kind, n, seed=n + run_len, dup=True)
+    if vals is None:
+        keys = workloads.sorted_runs(keys, run_len)
+    else:
+        keys, vals = workloads.sorted_runs(keys, run_len, vals)
+    splits = bcf.merge_partition(dev(keys), run_len, dev(vals)).cpu().numpy().view(np.uint32)
+    spp = -(-2 * run_len // 1024)
+    assert splits.size == bcf.num_shares(n, run_len)
+    for j, got in enumerate(splits):
+        pair, t = divmod(j, spp)
+        a0 = pair * 2 * run_len
+        a1 = min(n, a0 + run_len)
+        b1 = min(n, a1 + run_len)
+        d = min(t * 1024, b1 - a0)
+        want = oracle.corank(keys[a0:a1], keys[a1:b1], d,
+                             None if vals is None else vals[a0:a1], None if vals is None else vals[a1:b1])
+        assert got == want, (j, got, want)
+
+
+# ---------------------------------------------------------------- bcf_merge_runs (a6, a8, a9)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("n,run_len", [
+    (2048, 1024), (8192, 1024), (5000, 1024), (10000, 2048), (4097, 4096), (3000, 700),
+    (1 << 16, 1 << 12), (70001, 333), (1024, 1), (777, 1000), (1, 1), (2, 1), (40000, 20000), (40001, 13),
+])
+def test_merge_runs_matches_oracle(bcf, kind, n, run_len):
+    keys, vals = make(kind, n, seed=3 * n + run_len, dup=(n % 2 == 1))
+    if vals is None:
+        keys = workloads.sorted_runs(keys, run_len)
+    else:
+        keys, vals = workloads.sorted_runs(keys, run_len, vals)
+    dk, dv = dev(keys), dev(vals)
+    out = bcf.merge_runs(dk, run_len, dv)
+    want = oracle.merge_runs(keys, run_len, vals)
+    if vals is None:
+        assert np.array_equal(host(out, keys), want)
+    else:
+        assert np.array_equal(host(out[0], keys), want[0]) and np.array_equal(host(out[1], vals), want[1])
+    assert np.array_equal(host(dk, keys), keys)          # the input is not modified
+
+
+@pytest.mark.parametrize("k", [2, 64, 1024])
+def test_merge_runs_config5b_shape(bcf, k):
+    keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=1 << 18)
+    out = bcf.merge_runs(dev(keys), run_len)
+    assert np.array_equal(host(out, keys), oracle.merge_runs(keys, run_len))
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("n,run_len", [(2048, 1024), (9000, 1024), (5000, 700), (1 << 15, 512), (3, 1), (40001, 5000)])
+def test_merge_runs_pagewise_matches_oracle(bcf, kind, n, run_len):
+    """Row a7 (Alg. 6 streaming form): same unique result as the oracle's merge rounds, and the
+    oracle's own literal Alg. 6 on the first pair."""
+    keys, vals = make(kind, n, seed=n ^ run_len, dup=(n % 2 == 0))
+    if vals is None:
+        keys = workloads.sorted_runs(keys, run_len)
+    else:
+        keys, vals = workloads.sorted_runs(keys, run_len, vals)
+    out = bcf.merge_runs_pagewise(dev(keys), run_len, dev(vals))
+    want = oracle.merge_runs(keys, run_len, vals)
+    if vals is None:
+        assert np.array_equal(host(out, keys), want)
+    else:
+        assert np.array_equal(host(out[0], keys), want[0]) and np.array_equal(host(out[1], vals), want[1])
+    if n > 2 * run_len:   # one round only: compare with Alg. 6 itself on pair 0
+        a, b = keys[:run_len], keys[run_len:2 * run_len]
+        va = None if vals is None else vals[:run_len]
+        vb = None if vals is None else vals[run_len:2 * run_len]
+        one = bcf.merge_runs_pagewise(dev(np.concatenate([a, b])), run_len,
+                                      None if vals is None else dev(np.concatenate([va, vb])))
+        lit = oracle.binary_merge_pagewise(a, b, va, vb)
+        if vals is None:
+            assert np.array_equal(host(one, keys), lit)
+        else:
+            assert np.array_equal(host(one[0], keys), lit[0]) and np.array_equal(host(one[1], vals), lit[1])
+
+
+# ---------------------------------------------------------------- bcf_sort (a1-a9)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("n", [1, 2, 31, 1023, 1024, 1025, 2048, 5000, 3 * 1024 + 17, (1 << 16) + 17, 1 << 17])
+def test_sort_matches_oracle(bcf, kind, n):
+    keys, vals = make(kind, n, seed=n, dup=(n % 3 == 0))
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort(dk, dv)
+    want = oracle.sort_full(keys, vals)
+    assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+@pytest.mark.parametrize("dist", workloads.CFG4_VARIANTS)
+def test_sort_config4_distributions(bcf, dist):
+    keys = workloads.cfg4_sort_u32(dist, n=(1 << 18) + 1000)
+    d = dev(keys)
+    bcf.sort(d)
+    assert np.array_equal(host(d, keys), oracle.sort_full(keys))
+
+
+def test_sort_config3_and_5a_shapes(bcf):
+    keys = workloads.cfg3_sort_u32(n=1 << 19)
+    d = dev(keys)
+    bcf.sort(d)
+    assert np.array_equal(host(d, keys), oracle.sort_full(keys))
+    k, v = workloads.cfg5a_sort_u64_u32(n=(1 << 18) + 3)
+    dk, dv = dev(k), dev(v)
+    bcf.sort(dk, dv)
+    wk, wv = oracle.sort_full(k, v)
+    assert np.array_equal(host(dk, k), wk) and np.array_equal(host(dv, v), wv)
+
+
+def test_sort_empty_is_noop(bcf):
+    e = torch.empty(0, dtype=torch.int32, device="cuda")
+    bcf.sort(e)
+    bcf.sort_tiles(e)
+    assert bcf.merge_runs(e, 4).numel() == 0
+
+
+def test_sort_host_roundtrip(bcf):
+    keys, vals = make("u64u32", 50000, seed=1)
+    hk = torch.from_numpy(keys.view(np.int64).copy()).pin_memory()
+    hv = torch.from_numpy(vals.view(np.int32).copy()).pin_memory()
+    bcf.sort_host(hk, hv)
+    wk, wv = oracle.sort_full(keys, vals)
+    assert np.array_equal(hk.numpy().view(np.uint64), wk) and np.array_equal(hv.numpy().view(np.uint32), wv)
+
+
+# ---------------------------------------------------------------- error behaviour (include/bcf.h)
+
+
+def test_error_codes(bcf):
+    k = torch.zeros(4096, dtype=torch.int32, device="cuda")
+    with pytest.raises(bcf.BcfError) as e:
+        bcf.merge_runs(k, 0)
+    assert e.value.name == "BCF_ERR_INVALID_ARG"
+    with pytest.raises(bcf.BcfError) as e:
+        bcf.merge_runs(k, 1024, out_keys=k)                       # in/out aliasing
+    assert e.value.name == "BCF_ERR_INVALID_ARG"
+    with pytest.raises(bcf.BcfError) as e:
+        bcf.sort(k[1:])                                           # 4-byte aligned only
+    assert e.value.name == "BCF_ERR_MISALIGNED"
+    with pytest.raises(bcf.BcfError) as e:
+        bcf.sort(k, workspace=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    assert e.value.name == "BCF_ERR_WORKSPACE_TOO_SMALL"
+    with pytest.raises(ValueError):
+        bcf.sort(k.cpu())                                         # no CPU path
+
+
+def test_kernels_use_no_local_memory(bcf):
+    for cls in ("tile_sort", "partition", "merge"):
+        for kt in (0, 1):
+            for vt in (0, 1):
+                info = bcf.kernel_info(cls, kt, vt)
+                assert info["local_bytes_per_thread"] == 0, (cls, kt, vt, info)
+                assert info["ctas_per_sm"] >= 1
