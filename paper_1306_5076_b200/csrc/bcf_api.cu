@@ -8,6 +8,8 @@
 
 #include "bcf_kernels.cuh"
 #include "bcf_pagewise.cuh"
+#include "bcf_merge_pipe.cuh"
+#include <cstdlib>
 
 using namespace bcf;
 
@@ -161,6 +163,49 @@ bcf_status launch_merge(const void *kin, const uint32_t *vin, void *kout, uint32
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }
 
+// Power-of-two multiples of the tile size take the pipelined kernel (bcf_merge_pipe.cuh).
+inline bool pipe_eligible(size_t run_len)
+{
+    if (run_len % TILE) return false;
+    const size_t r = run_len / TILE;
+    if (r & (r - 1)) return false;
+    static int forced_v1 = -1;
+    if (forced_v1 < 0) {
+        const char *e = std::getenv("BCF_MERGE_IMPL");
+        forced_v1 = (e && std::strcmp(e, "v1") == 0) ? 1 : 0;
+    }
+    return !forced_v1;
+}
+
+bcf_status launch_merge_pipe(const uint32_t *kin, uint32_t *kout, uint32_t *splits, size_t n, size_t run_len,
+                             cudaStream_t s)
+{
+    const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
+    if (shares == 0) return BCF_OK;
+    static int num_sms = 0;
+    if (!num_sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return BCF_ERR_CUDA;
+        if (cudaFuncSetAttribute(pipe::merge_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)pipe::SmemLayout::total) != cudaSuccess)
+            return BCF_ERR_CUDA;
+    }
+    if (2 * run_len > (size_t)pipe::SH) {
+        LaunchTimer t(BCF_KERNEL_PARTITION, s);
+        const unsigned blocks = static_cast<unsigned>((shares + 1 + 127) / 128);
+        pipe::partition_share_kernel<<<blocks, 128, 0, s>>>(kin, splits, n, run_len, shares);
+    }
+    {
+        LaunchTimer t(BCF_KERNEL_MERGE, s);
+        const unsigned long long cap = 2ull * num_sms;
+        const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
+        pipe::merge_pipe_kernel<<<blocks, pipe::THREADS, pipe::SmemLayout::total, s>>>(kin, kout, splits, n, run_len, shares);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
 template <class E>
 bcf_status launch_pagewise(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, size_t run_len,
                            cudaStream_t s)
@@ -228,7 +273,18 @@ bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *
         const PassGeom g = pass_geom(n, l);
         void *kd = to_a ? ka : kb;
         uint32_t *vd = to_a ? va : vb;
-        bcf_status st = launch_partition<E>(ksrc, vsrc, splits, g, s);
+        bcf_status st;
+        if constexpr (E::NP == 1) {
+            if (pipe_eligible(l)) {
+                st = launch_merge_pipe(static_cast<const uint32_t *>(ksrc), static_cast<uint32_t *>(kd), splits, n, l, s);
+                if (st != BCF_OK) return st;
+                ksrc = kd;
+                vsrc = vd;
+                to_a = !to_a;
+                continue;
+            }
+        }
+        st = launch_partition<E>(ksrc, vsrc, splits, g, s);
         if (st != BCF_OK) return st;
         st = launch_merge<E>(ksrc, vsrc, kd, vd, splits, g, s);
         if (st != BCF_OK) return st;
