@@ -19,19 +19,84 @@ constexpr uint32_t SENTINEL = 0xFFFFFFFFu;   // "infinity" in every plane (PAPER
 
 // ------------------------------------------------------------------ global memory access
 
+// Every element is read once and written once per kernel: allocating those lines in L1 buys
+// nothing, and the L1 data array is the SAME SRAM as shared memory, so L1 fills and write-through
+// data compete with the warps' shared-memory wavefronts for its 32 banks.  Loads therefore carry
+// L1::no_allocate and stores are streaming (.cs).  BCF_GMEM_HINT=0 restores the default policies
+// (kept for the A/B measurement recorded in profiles/).
+#ifndef BCF_GMEM_HINT
+#define BCF_GMEM_HINT 1
+#endif
+
+__device__ __forceinline__ uint4 ldg128(const uint4 *p)
+{
+#if BCF_GMEM_HINT
+    uint4 t;
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(t.x), "=r"(t.y), "=r"(t.z), "=r"(t.w) : "l"(p));
+    return t;
+#else
+    return *p;
+#endif
+}
+__device__ __forceinline__ uint2 ldg64(const uint2 *p)
+{
+#if BCF_GMEM_HINT
+    uint2 t;
+    asm volatile("ld.global.L1::no_allocate.v2.u32 {%0, %1}, [%2];" : "=r"(t.x), "=r"(t.y) : "l"(p));
+    return t;
+#else
+    return *p;
+#endif
+}
+__device__ __forceinline__ uint32_t ldg32(const uint32_t *p)
+{
+#if BCF_GMEM_HINT
+    uint32_t t;
+    asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(t) : "l"(p));
+    return t;
+#else
+    return *p;
+#endif
+}
+__device__ __forceinline__ void stg128(uint4 *p, const uint4 t)
+{
+#if BCF_GMEM_HINT
+    __stcs(p, t);
+#else
+    *p = t;
+#endif
+}
+__device__ __forceinline__ void stg64(uint2 *p, const uint2 t)
+{
+#if BCF_GMEM_HINT
+    __stcs(p, t);
+#else
+    *p = t;
+#endif
+}
+__device__ __forceinline__ void stg32(uint32_t *p, const uint32_t t)
+{
+#if BCF_GMEM_HINT
+    __stcs(p, t);
+#else
+    *p = t;
+#endif
+}
+
 // Element `g` of the SoA arrays into planes of register slot k.
 template <class E>
 __device__ __forceinline__ void load_elem(const void *keys, const uint32_t *vals, const size_t g,
                                           uint32_t (&v)[E::NP][32], const int k)
 {
     if constexpr (E::KEY_WORDS == 1) {
-        v[0][k] = static_cast<const uint32_t *>(keys)[g];
+        v[0][k] = ldg32(static_cast<const uint32_t *>(keys) + g);
     } else {
-        const uint2 t = reinterpret_cast<const uint2 *>(keys)[g];
+        const uint2 t = ldg64(reinterpret_cast<const uint2 *>(keys) + g);
         v[0][k] = t.y;   // high word first: planes are compared in order
         v[1][k] = t.x;
     }
-    if constexpr (E::HAS_VAL) v[E::KEY_WORDS][k] = vals[g];
+    if constexpr (E::HAS_VAL) v[E::KEY_WORDS][k] = ldg32(vals + g);
 }
 
 template <class E>
@@ -52,14 +117,14 @@ __device__ __forceinline__ void load_tile_vec(const void *keys, const uint32_t *
         const uint4 *pk = reinterpret_cast<const uint4 *>(static_cast<const uint32_t *>(keys) + base);
 #pragma unroll
         for (int m = 0; m < 8; ++m) {
-            const uint4 t = pk[32 * m + lane];
+            const uint4 t = ldg128(pk + 32 * m + lane);
             v[0][4 * m] = t.x; v[0][4 * m + 1] = t.y; v[0][4 * m + 2] = t.z; v[0][4 * m + 3] = t.w;
         }
         if constexpr (E::HAS_VAL) {
             const uint4 *pv = reinterpret_cast<const uint4 *>(vals + base);
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
-                const uint4 t = pv[32 * m + lane];
+                const uint4 t = ldg128(pv + 32 * m + lane);
                 v[1][4 * m] = t.x; v[1][4 * m + 1] = t.y; v[1][4 * m + 2] = t.z; v[1][4 * m + 3] = t.w;
             }
         }
@@ -67,14 +132,14 @@ __device__ __forceinline__ void load_tile_vec(const void *keys, const uint32_t *
         const uint4 *pk = reinterpret_cast<const uint4 *>(static_cast<const uint64_t *>(keys) + base);
 #pragma unroll
         for (int m = 0; m < 16; ++m) {
-            const uint4 t = pk[32 * m + lane];   // keys 64m + 2 lane, +1
+            const uint4 t = ldg128(pk + 32 * m + lane);   // keys 64m + 2 lane, +1
             v[0][2 * m] = t.y; v[1][2 * m] = t.x; v[0][2 * m + 1] = t.w; v[1][2 * m + 1] = t.z;
         }
         if constexpr (E::HAS_VAL) {
             const uint2 *pv = reinterpret_cast<const uint2 *>(vals + base);
 #pragma unroll
             for (int m = 0; m < 16; ++m) {
-                const uint2 t = pv[32 * m + lane];
+                const uint2 t = ldg64(pv + 32 * m + lane);
                 v[2][2 * m] = t.x; v[2][2 * m + 1] = t.y;
             }
         }
@@ -113,14 +178,14 @@ __device__ __forceinline__ void store_rows(uint32_t *planes, void *keys, uint32_
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
                 const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
-                pk[32 * m + lane] = *reinterpret_cast<const uint4 *>(planes + w);
+                stg128(pk + 32 * m + lane, *reinterpret_cast<const uint4 *>(planes + w));
             }
             if constexpr (E::HAS_VAL) {
                 uint4 *pv = reinterpret_cast<uint4 *>(vals + base);
 #pragma unroll
                 for (int m = 0; m < 8; ++m) {
                     const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
-                    pv[32 * m + lane] = *reinterpret_cast<const uint4 *>(planes + TILE + w);
+                    stg128(pv + 32 * m + lane, *reinterpret_cast<const uint4 *>(planes + TILE + w));
                 }
             }
         } else {
@@ -130,14 +195,14 @@ __device__ __forceinline__ void store_rows(uint32_t *planes, void *keys, uint32_
                 const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
                 const uint2 hi = *reinterpret_cast<const uint2 *>(planes + w);
                 const uint2 lo = *reinterpret_cast<const uint2 *>(planes + TILE + w);
-                pk[32 * m + lane] = make_uint4(lo.x, hi.x, lo.y, hi.y);
+                stg128(pk + 32 * m + lane, make_uint4(lo.x, hi.x, lo.y, hi.y));
             }
             if constexpr (E::HAS_VAL) {
                 uint2 *pv = reinterpret_cast<uint2 *>(vals + base);
 #pragma unroll
                 for (int m = 0; m < 16; ++m) {
                     const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
-                    pv[32 * m + lane] = *reinterpret_cast<const uint2 *>(planes + 2 * TILE + w);
+                    stg64(pv + 32 * m + lane, *reinterpret_cast<const uint2 *>(planes + 2 * TILE + w));
                 }
             }
         }
@@ -148,11 +213,11 @@ __device__ __forceinline__ void store_rows(uint32_t *planes, void *keys, uint32_
                 const int w = elem_word(k, lane);
                 const size_t g = base + 32 * k + lane;
                 if constexpr (E::KEY_WORDS == 1) {
-                    static_cast<uint32_t *>(keys)[g] = planes[w];
+                    stg32(static_cast<uint32_t *>(keys) + g, planes[w]);
                 } else {
-                    reinterpret_cast<uint2 *>(keys)[g] = make_uint2(planes[TILE + w], planes[w]);
+                    stg64(reinterpret_cast<uint2 *>(keys) + g, make_uint2(planes[TILE + w], planes[w]));
                 }
-                if constexpr (E::HAS_VAL) vals[g] = planes[E::KEY_WORDS * TILE + w];
+                if constexpr (E::HAS_VAL) stg32(vals + g, planes[E::KEY_WORDS * TILE + w]);
             }
         }
     }
