@@ -36,18 +36,107 @@ from paper_1306_5076_b200 import workloads  # noqa: E402
 
 METRIC = "sorted keys/sec"
 UNIT = "keys/s"
+
+
+def _keys_only(gen):
+    return lambda n: (gen(n), None)
+
+
+# name: (description, default log2 n, generator(n) -> (keys, vals), op, dtype)
+#   op = "sort" (bcf_sort), "tiles" (bcf_sort_tiles) or ("merge", k) (bcf_merge_runs on k equal sorted runs)
 WORKLOADS = {
-    # name: (description, log2 n default, generator)
     "cfg4a": ("BCFMergesort of 2^28 uint32 keys, uniform over [0,2^32) (BASELINE.json config 4, uniform)", 28,
-              lambda n: workloads.cfg4_sort_u32("uniform", n=n)),
-    "cfg4b": ("config 4, already sorted", 28, lambda n: workloads.cfg4_sort_u32("sorted", n=n)),
-    "cfg4c": ("config 4, reverse sorted", 28, lambda n: workloads.cfg4_sort_u32("reverse", n=n)),
-    "cfg4d": ("config 4, 256 distinct values", 28, lambda n: workloads.cfg4_sort_u32("dup256", n=n)),
-    "cfg4e": ("config 4, Zipf(1.1) over [0,2^20)", 28, lambda n: workloads.cfg4_sort_u32("zipf", n=n)),
-    "cfg3": ("BCFMergesort of 2^24 uint32 keys, uniform (BASELINE.json config 3)", 24,
-             lambda n: workloads.cfg3_sort_u32(n=n)),
+              _keys_only(lambda n: workloads.cfg4_sort_u32("uniform", n=n)), "sort", "u32"),
+    "cfg4b": ("config 4, already sorted", 28, _keys_only(lambda n: workloads.cfg4_sort_u32("sorted", n=n)), "sort", "u32"),
+    "cfg4c": ("config 4, reverse sorted", 28, _keys_only(lambda n: workloads.cfg4_sort_u32("reverse", n=n)), "sort", "u32"),
+    "cfg4d": ("config 4, 256 distinct values", 28, _keys_only(lambda n: workloads.cfg4_sort_u32("dup256", n=n)), "sort", "u32"),
+    "cfg4e": ("config 4, Zipf(1.1) over [0,2^20)", 28, _keys_only(lambda n: workloads.cfg4_sort_u32("zipf", n=n)), "sort", "u32"),
+    "cfg3": ("BCFMergesort of 2^24 uint32 keys, uniform (BASELINE.json config 3; fits the L2)", 24,
+             _keys_only(lambda n: workloads.cfg3_sort_u32(n=n)), "sort", "u32"),
+    "cfg1": ("batch tile sort, 1024 tiles of 32x32 uint32 (BASELINE.json config 1; latency-bound)", 20,
+             _keys_only(lambda n: workloads.cfg1_tiles_u32(num_tiles=n // 1024)), "tiles", "u32"),
+    "cfg2": ("batch tile sort, 2^16 tiles of (u32 key in [0,16), u32 value = index) (BASELINE.json config 2)", 26,
+             lambda n: workloads.cfg2_tiles_u32_u32(num_tiles=n // 1024), "tiles", "u32+u32"),
+    "cfg5a": ("key-value BCFMergesort of 2^26 (u64 key, u32 value) pairs (BASELINE.json config 5)", 26,
+              lambda n: workloads.cfg5a_sort_u64_u32(n=n), "sort", "u64+u32"),
+    "cfg5b2": ("merge-only, 2 sorted uint32 runs totalling 2^27 keys (config 5)", 27, None, ("merge", 2), "u32"),
+    "cfg5b64": ("merge-only, 64 sorted uint32 runs totalling 2^27 keys (config 5)", 27, None, ("merge", 64), "u32"),
+    "cfg5b1024": ("merge-only, 1024 sorted uint32 runs totalling 2^27 keys (config 5)", 27, None, ("merge", 1024), "u32"),
 }
-ORACLE_SAMPLE_LOG2 = 25   # ~15 s of single-thread CPU work
+SIDE_WORKLOADS = ("cfg1", "cfg2", "cfg3", "cfg5a", "cfg5b64")   # short device-timed lines beside the headline
+ORACLE_SAMPLE_LOG2 = 25   # ~6 s of single-thread CPU work
+
+
+def elem_bytes(dtype):
+    return {"u32": 4, "u32+u32": 8, "u64": 8, "u64+u32": 12}[dtype]
+
+
+def make_input(name, n):
+    """(keys, vals, run_len) host arrays of workload `name` at n elements."""
+    desc, logn, gen, op, dtype = WORKLOADS[name]
+    if isinstance(op, tuple):
+        keys, run_len = workloads.cfg5b_merge_runs_u32(op[1], n=n)
+        return keys, None, run_len
+    keys, vals = gen(n)
+    return keys, vals, 0
+
+
+class Job:
+    """One workload resident on the device: restore() the pristine input, run() one step."""
+
+    def __init__(self, bcf, torch, dev, name, n, rank=0):
+        desc, logn, gen, op, dtype = WORKLOADS[name]
+        self.name, self.desc, self.op, self.dtype, self.n = name, desc, op, dtype, n
+        keys, vals, self.run_len = make_input(name, n)
+        if rank:
+            keys = replica_keys(keys, rank, sorted_runs=self.run_len)
+        self.host_keys, self.host_vals = keys, vals
+        signed = {np.dtype(np.uint32): np.int32, np.dtype(np.uint64): np.int64}
+        self.src_k = torch.from_numpy(keys.view(signed[keys.dtype])).to(dev)
+        self.src_v = None if vals is None else torch.from_numpy(vals.view(np.int32)).to(dev)
+        self.k = torch.empty_like(self.src_k)
+        self.v = None if vals is None else torch.empty_like(self.src_v)
+        self.bcf = bcf
+        kt = bcf.binding.BCF_KEY_U64 if keys.dtype == np.uint64 else bcf.binding.BCF_KEY_U32
+        vt = bcf.binding.BCF_VAL_NONE if vals is None else bcf.binding.BCF_VAL_U32
+        if op == "sort":
+            need = bcf.workspace_bytes(bcf.binding.OP_SORT, n, kt=kt, vt=vt)
+        elif op == "tiles":
+            need = 0
+        else:
+            need = bcf.workspace_bytes(bcf.binding.OP_MERGE_RUNS, n, self.run_len, kt=kt, vt=vt)
+            self.out_k = torch.empty_like(self.src_k)
+        self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+        self.passes = None
+
+    def restore(self):
+        if self.op in ("sort", "tiles"):
+            self.k.copy_(self.src_k)
+            if self.v is not None:
+                self.v.copy_(self.src_v)
+
+    def run(self):
+        b = self.bcf
+        if self.op == "sort":
+            b.sort(self.k, self.v, workspace=self.ws)
+        elif self.op == "tiles":
+            b.sort_tiles(self.k, self.v)
+        else:
+            b.merge_runs(self.src_k, self.run_len, out_keys=self.out_k, workspace=self.ws)
+
+    def result(self):
+        return self.out_k if isinstance(self.op, tuple) else self.k
+
+    def check(self):
+        """Cheap any-size property of the result (the parity tests do the real comparison)."""
+        out = self.result().cpu().numpy().view(self.host_keys.dtype)
+        if self.op == "tiles":
+            t = out.reshape(-1, 1024)
+            ok = bool(np.all(t[:, :-1] <= t[:, 1:]))
+        else:
+            ok = bool(np.all(out[:-1] <= out[1:]))
+        if not ok:
+            raise SystemExit(f"bench: output of {self.name} not sorted")
 
 
 def measured_peak():
@@ -120,12 +209,12 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def replica_keys(keys, rank):
+def replica_keys(keys, rank, sorted_runs=0):
     """Replicas only: rank r sorts the same recipe, rotated and re-keyed so that no two ranks share
-    an input (the multiset differs, the distribution does not)."""
-    if rank == 0:
+    an input (the multiset differs, the distribution does not).  Pre-sorted runs stay as they are."""
+    if rank == 0 or sorted_runs:
         return keys
-    return np.roll(keys, 7919 * rank) ^ np.uint32(rank)
+    return np.roll(keys, 7919 * rank) ^ keys.dtype.type(rank)
 
 
 def max_over_ranks(ms, world, device=None):
@@ -139,33 +228,96 @@ def max_over_ranks(ms, world, device=None):
     return float(t.item())
 
 
+def oracle_run(name, keys, vals, run_len):
+    """The CPU oracle on one host input of workload `name`; returns seconds."""
+    import oracle
+    op = WORKLOADS[name][3]
+    t0 = time.perf_counter()
+    if op == "sort":
+        out = oracle.sort_full(keys, vals)
+    elif op == "tiles":
+        out = oracle.shearsort_tiles(keys, vals)
+    else:
+        out = oracle.merge_runs(keys, run_len)
+    dt = time.perf_counter() - t0
+    k = out if vals is None else out[0]
+    if op != "tiles":
+        assert np.all(k[:-1] <= k[1:])
+    return dt
+
+
+def oracle_sample(name, n_full):
+    """A bounded sample of the workload for the CPU legs: the first 2^25 elements of the same recipe
+    (whole tiles / whole runs), about 5-10 s of single-thread work."""
+    op = WORKLOADS[name][3]
+    n = min(n_full, 1 << ORACLE_SAMPLE_LOG2)
+    keys, vals, run_len = make_input(name, n)
+    what = {"sort": "oracle.sort_full (ShearSort 32x32 tiles + two-finger merge rounds)",
+            "tiles": "oracle.shearsort_tiles"}.get(op, "oracle.merge_runs (two-finger merge rounds)")
+    return keys, vals, run_len, n, f"{what} on the first 2^{int(np.log2(n))} elements of the workload recipe, 1 thread"
+
+
 def run_reference(args, rank, world):
     """This tier's reference arm: the CPU oracle as it stands, on a bounded sample per step."""
     if rank != 0:
         return
-    import oracle
-    desc, logn, gen = WORKLOADS[args.workload]
+    desc, logn, gen, op, dtype = WORKLOADS[args.workload]
     n_full = 1 << (args.log2n or logn)
-    n = min(n_full, 1 << ORACLE_SAMPLE_LOG2)
-    keys = gen(n)   # same recipe and stream: the first n draws of the workload
-    for _ in range(args.warmup and 1):
-        oracle.sort_full(keys[: 1 << 16])
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        out = oracle.sort_full(keys)
-    dt = time.perf_counter() - t0
-    assert np.all(out[:-1] <= out[1:])
+    keys, vals, run_len, n, sample = oracle_sample(args.workload, n_full)
+    if args.warmup:
+        oracle_run(args.workload, keys[: 1 << 12], None if vals is None else vals[: 1 << 12], min(run_len, 1 << 11))
+    dt = sum(oracle_run(args.workload, keys, vals, run_len) for _ in range(args.steps))
     value = n * args.steps / dt
-    sample = f"oracle.sort_full (ShearSort 32x32 tiles + two-finger merge rounds) on the first 2^{int(np.log2(n))} keys of the workload, per step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "n": n_full, "sample_n": n},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample + ", per step"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
+
+
+def time_steps(torch, job, steps, stream, barrier):
+    """Device time (ms) of `steps` steps: CUDA events around each call on the launching stream; the
+    restore copy of the pristine input is outside the events."""
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier()
+    for a, b in ev:
+        job.restore()
+        a.record(stream)
+        job.run()
+        b.record(stream)
+    barrier()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
+def side_line(bcf, torch, dev, name, stream, barrier):
+    """A short device-timed measurement of another BASELINE.json config (3 warm-ups, 5 steps)."""
+    desc, logn, gen, op, dtype = WORKLOADS[name]
+    n = 1 << logn
+    job = Job(bcf, torch, dev, name, n)
+    for _ in range(3):
+        job.restore()
+        job.run()
+    torch.cuda.synchronize()
+    job.check()
+    bcf.launch_counts()
+    ms = time_steps(torch, job, 5, stream, barrier)
+    launches = bcf.launch_counts()
+    t = sum(ms) / len(ms)
+    rounds = (launches["merge"] + launches["merge_pagewise"]) // 5
+    passes = rounds + (0 if isinstance(op, tuple) else 1)
+    bytes_moved = passes * 2 * elem_bytes(dtype) * n
+    peak, _ = measured_peak()
+    line = {"workload": name, "description": desc, "dtype": dtype, "n": n, "value": n / (t * 1e-3), "unit": UNIT,
+            "ms_per_step": t, "best_ms": min(ms), "passes": passes,
+            "frac_of_measured_hbm_peak_for_pass_count": bytes_moved / (t * 1e-3) / 1e9 / peak,
+            "gpu_launches_per_step": int(sum(launches.values())) // 5}
+    del job
+    torch.cuda.empty_cache()
+    return line
 
 
 def main():
@@ -178,6 +330,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=0, help="override the element count (debugging only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-side", action="store_true", help="skip the short lines for the other configs")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -186,7 +339,7 @@ def main():
 
     if args.impl == "reference":
         if args.steps > 3:
-            args.steps = 3           # bounded: each step is ~15 s of CPU
+            args.steps = 3           # bounded: each step is several seconds of CPU
         run_reference(args, rank, world)
         return
 
@@ -203,13 +356,11 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
 
-    desc, logn, gen = WORKLOADS[args.workload]
+    desc, logn, gen, op, dtype = WORKLOADS[args.workload]
     n = 1 << (args.log2n or logn)
-    # replicas only: every rank sorts its own n keys (rank r draws from variant stream r for cfg3/4a)
-    keys = replica_keys(gen(n), rank)
-    src = torch.from_numpy(keys.view(np.int32)).to(dev)
-    work = torch.empty_like(src)
-    ws = torch.empty(bcf.workspace_bytes(bcf.binding.OP_SORT, n), dtype=torch.uint8, device=dev)
+    eb = elem_bytes(dtype)
+    # replicas only: every rank works on its own n elements of the same recipe
+    job = Job(bcf, torch, dev, args.workload, n, rank)
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -218,111 +369,123 @@ def main():
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        work.copy_(src)
-        bcf.sort(work, workspace=ws)
+        job.restore()
+        job.run()
     torch.cuda.synchronize()
-    out = work.cpu().numpy().view(np.uint32)
-    if not np.all(out[:-1] <= out[1:]):
-        raise SystemExit("bench: output not sorted")
-    del out
+    job.check()
 
     # ---------------- timed region: K steps, device-timed
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     sampler = ClockSampler(local_rank)
     bcf.launch_counts()
     bcf.profile_enable(True)
-    barrier()
     sampler.start()
     t_wall = time.perf_counter()
-    for a, b in ev:
-        work.copy_(src)              # restore the unsorted input (outside the events)
-        a.record(stream)
-        bcf.sort(work, workspace=ws)
-        b.record(stream)
-    barrier()
+    step_ms = time_steps(torch, job, args.steps, stream, barrier)
     t_wall = time.perf_counter() - t_wall
     clocks = sampler.stop()
     prof = bcf.profile_read()
     bcf.profile_enable(False)
     launches = bcf.launch_counts()
-    ms = sum(a.elapsed_time(b) for a, b in ev)
-    ms = max_over_ranks(ms, world, dev)
+    ms = max_over_ranks(sum(step_ms), world, dev)
     value = world * n * args.steps / (ms * 1e-3)
 
-    # ---------------- roofline of the dominant kernel (merge), same timed region
+    # ---------------- roofline of the dominant kernel, same timed region
     peak, peak_src = measured_peak()
-    m_ms, m_cnt = prof["merge"]
-    rounds = m_cnt // max(args.steps, 1)
-    alg_bytes = 2 * 4 * n
-    achieved = alg_bytes / (m_ms / m_cnt * 1e-3) / 1e9 if m_cnt else None
-    roofline = {
-        "kernel": "merge_kernel<u32> (one launch = one merge round: read + write all n keys)",
-        "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-        "frac": achieved / peak if achieved else None, "traffic": recorded_traffic("merge"),
-        "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-        "launches_timed": m_cnt, "mean_launch_ms": m_ms / m_cnt if m_cnt else None,
-        "share_of_step": {k: v[0] / ms for k, v in prof.items() if v[1]},
-        "whole_sort": {
-            "passes": 1 + rounds,
-            "frac_of_measured_peak": (1 + rounds) * alg_bytes / (ms / args.steps * 1e-3) / 1e9 / peak,
-            "frac_of_nominal_8TBps": (1 + rounds) * alg_bytes / (ms / args.steps * 1e-3) / 1e9 / 8000.0,
-        },
-    }
+    dom = max((k for k in prof if prof[k][1]), key=lambda k: prof[k][0])
+    d_ms, d_cnt = prof[dom]
+    rounds = (prof["merge"][1] + prof["merge_pagewise"][1]) // max(args.steps, 1)
+    passes = rounds + (0 if isinstance(op, tuple) else 1)
+    alg_bytes = 2 * eb * n
+    share = {k: v[0] / ms for k, v in prof.items() if v[1]}
+    if dom == "tile_sort" and op == "tiles":
+        # ALU-bound: 11 line sorts x 191 comparators x 2 min/max per 32 u32 keys,
+        # integer min/max issue at 64 lanes / clk / SM.
+        sm_mhz = clocks.get("sm_max_mhz") or 1965.0
+        ops = n * 11 * 191 * 2 / 32 * {"u32": 1, "u32+u32": 5, "u64": 5, "u64+u32": 8}[dtype]
+        peak_ops = 148 * 64 * sm_mhz * 1e6
+        ach = ops / (d_ms / d_cnt * 1e-3)
+        roofline = {"kernel": "tile_sort_kernel (one launch = ShearSort of all tiles)", "bound": "alu",
+                    "achieved": ach / 1e12, "peak": peak_ops / 1e12, "unit": "T int-op/s", "frac": ach / peak_ops,
+                    "traffic": recorded_traffic("tile_sort"),
+                    "peak_source": "148 SMs x 64 integer min/max lanes per clk x SM max clock (DESIGN.md 5.1)",
+                    "launches_timed": d_cnt, "mean_launch_ms": d_ms / d_cnt, "share_of_step": share}
+    else:
+        m_ms, m_cnt = prof["merge"]
+        achieved = alg_bytes / (m_ms / m_cnt * 1e-3) / 1e9 if m_cnt else None
+        roofline = {
+            "kernel": "merge kernel (one launch = one merge round: read + write all n elements)",
+            "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak if achieved else None, "traffic": recorded_traffic("merge"),
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+            "launches_timed": m_cnt, "mean_launch_ms": m_ms / m_cnt if m_cnt else None,
+            "share_of_step": share,
+            "whole_step": {
+                "passes": passes,
+                "frac_of_measured_peak": passes * alg_bytes / (ms / args.steps * 1e-3) / 1e9 / peak,
+                "frac_of_nominal_8TBps": passes * alg_bytes / (ms / args.steps * 1e-3) / 1e9 / 8000.0,
+            },
+        }
 
     # ---------------- e2e: host buffers through bcf_sort_host, copies inside the timed region
     e2e = None
-    if not args.no_e2e:
-        hsrc = torch.from_numpy(keys.view(np.int32))
-        hbuf = torch.empty_like(hsrc).pin_memory()
-        scratch = torch.empty(bcf.workspace_bytes(bcf.binding.OP_SORT_HOST, n), dtype=torch.uint8, device=dev)
+    if not args.no_e2e and op == "sort":
+        hk_src = torch.from_numpy(job.host_keys.view(np.int64 if job.host_keys.dtype == np.uint64 else np.int32))
+        hk = torch.empty_like(hk_src).pin_memory()
+        hv_src = None if job.host_vals is None else torch.from_numpy(job.host_vals.view(np.int32))
+        hv = None if hv_src is None else torch.empty_like(hv_src).pin_memory()
+        kt = bcf.binding.BCF_KEY_U64 if job.host_keys.dtype == np.uint64 else bcf.binding.BCF_KEY_U32
+        vt = bcf.binding.BCF_VAL_NONE if hv is None else bcf.binding.BCF_VAL_U32
+        scratch = torch.empty(bcf.workspace_bytes(bcf.binding.OP_SORT_HOST, n, kt=kt, vt=vt), dtype=torch.uint8, device=dev)
         e_steps = max(1, min(args.steps, 5))
         e_ms = 0.0
         for i in range(1 + e_steps):
-            hbuf.copy_(hsrc)
+            hk.copy_(hk_src)
+            if hv is not None:
+                hv.copy_(hv_src)
             barrier()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
-            bcf.sort_host(hbuf, scratch=scratch)
+            bcf.sort_host(hk, hv, scratch=scratch)
             b.record(stream)
             torch.cuda.synchronize()
             if i:
                 e_ms += a.elapsed_time(b)
         e_ms = max_over_ranks(e_ms, world, dev)
         e2e = {"value": world * n * e_steps / (e_ms * 1e-3), "unit": UNIT, "steps": e_steps,
-               "h2d_bytes_per_step": 4 * n, "d2h_bytes_per_step": 4 * n,
-               "api": "bcf_sort_host (pinned host buffer; H2D + sort + D2H + stream sync inside the timed region)"}
-        hk = hbuf.numpy().view(np.uint32)
-        if not np.all(hk[:-1] <= hk[1:]):
+               "h2d_bytes_per_step": eb * n, "d2h_bytes_per_step": eb * n,
+               "api": "bcf_sort_host (pinned host buffers; H2D + sort + D2H + stream sync inside the timed region)"}
+        out = hk.numpy().view(job.host_keys.dtype)
+        if not np.all(out[:-1] <= out[1:]):
             raise SystemExit("bench: e2e output not sorted")
-        del scratch, hbuf
+        del scratch, hk, hv
 
-    # ---------------- CPU oracle beside it (rank 0, N = 1 only)
+    # ---------------- CPU oracle beside it, and the other configs (rank 0, N = 1 only)
     cpu = None
+    side = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        import oracle
-        sn = min(n, 1 << ORACLE_SAMPLE_LOG2)
-        sample = keys[:sn].copy()
-        t0 = time.perf_counter()
-        so = oracle.sort_full(sample)
-        dt = time.perf_counter() - t0
-        assert np.all(so[:-1] <= so[1:])
+        keys, vals, run_len, sn, sample = oracle_sample(args.workload, n)
+        dt = oracle_run(args.workload, keys, vals, run_len)
         cpu = {"value": sn / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
-               "host_cores_total": os.cpu_count(),
-               "sample": f"oracle.sort_full on the first 2^{int(np.log2(sn))} keys of the same workload, once"}
+               "host_cores_total": os.cpu_count(), "sample": sample + ", once"}
+    if rank == 0 and world == 1 and not args.no_side and args.workload == "cfg4a" and not args.log2n:
+        del job
+        torch.cuda.empty_cache()
+        side = [side_line(bcf, torch, dev, w, stream, barrier) for w in SIDE_WORKLOADS]
 
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-            "config": {"workload": args.workload, "description": desc, "n": n, "bytes": 4 * n,
-                       "passes": 1 + rounds, "multi_gpu": "replicas only",
-                       "l2": "input (4*n bytes = 1 GiB at n = 2^28) and workspace are larger than the 126 MB L2; "
-                             "the input is restored from a pristine copy before every step",
-                       "timing": "CUDA events around each bcf_sort call; restore copy outside the events",
-                       "wall_s_timed_region": t_wall},
+            "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+            "config": {"workload": args.workload, "description": desc, "n": n, "bytes": eb * n,
+                       "passes": passes, "multi_gpu": "replicas only",
+                       "l2": "input and workspace (%d MiB each) %s the 126 MB L2; the input is restored from a "
+                             "pristine copy before every step" % (eb * n >> 20, "exceed" if eb * n > 126e6 else "FIT IN"),
+                       "timing": "CUDA events around each library call; restore copy outside the events",
+                       "best_step_ms": min(step_ms), "wall_s_timed_region": t_wall},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(launches.values())),
             "launches_by_kernel": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "other_workloads": side,
         }))
     if world > 1:
         dist.destroy_process_group()
