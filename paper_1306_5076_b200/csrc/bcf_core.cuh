@@ -29,6 +29,56 @@ struct Elem {
 };
 
 // ------------------------------------------------------------------ compare-exchange
+//
+// Pipe balance (measured on B200): integer min/max, compare, select and add/sub with
+// carry all issue on the ALU pipe (16 lanes / clk / SM sub-partition), integer multiply-add on the
+// FMA pipe.  A compare-exchange written with ALU instructions only leaves the FMA pipe idle, so part
+// of the "larger" outputs are formed as  hi = a + b - lo  (mod 2^32, exact) with two IMADs whose
+// multiplier comes from constant memory -- opaque to ptxas, which would otherwise turn them back
+// into ALU adds.
+__constant__ uint32_t c_one = 1u;
+__constant__ uint32_t c_minus_one = 0xFFFFFFFFu;
+
+// a + b - lo on the FMA pipe (lo is one of a, b; the result is the other one).
+__device__ __forceinline__ uint32_t other_of(const uint32_t a, const uint32_t b, const uint32_t lo)
+{
+    uint32_t s, hi;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(s) : "r"(a), "r"(c_one), "r"(b));
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(hi) : "r"(lo), "r"(c_minus_one), "r"(s));
+    return hi;
+}
+
+// x > y for elements of NP planes compared lexicographically: one subtract-with-borrow chain from
+// the least significant plane up (NP ALU instructions).
+template <int NP>
+__device__ __forceinline__ bool elem_gt(const uint32_t (&v)[NP][32], const int i, const int j)
+{
+    uint32_t bo;
+    if constexpr (NP == 2) {
+        asm("{\n .reg .u32 t;\n sub.cc.u32 t, %2, %1;\n subc.cc.u32 t, %4, %3;\n subc.u32 %0, 0, 0;\n}"
+            : "=r"(bo) : "r"(v[1][i]), "r"(v[1][j]), "r"(v[0][i]), "r"(v[0][j]));
+    } else {
+        asm("{\n .reg .u32 t;\n sub.cc.u32 t, %2, %1;\n subc.cc.u32 t, %4, %3;\n subc.cc.u32 t, %6, %5;\n"
+            " subc.u32 %0, 0, 0;\n}"
+            : "=r"(bo) : "r"(v[2][i]), "r"(v[2][j]), "r"(v[1][i]), "r"(v[1][j]), "r"(v[0][i]), "r"(v[0][j]));
+    }
+    return bo != 0;
+}
+
+// Tuning knobs (A/B measured on B200 in the real kernels, where register pressure limits what the
+// micro-benchmark promises; the defaults are the fastest):
+//   BCF_CE1_FMA_MOD     keys-only: comparator (i, j) forms its max on the FMA pipe when i % MOD != 0 (0: never)
+//   BCF_CE2_FMA_PLANES  two-plane elements: the last this-many planes form their "larger" output on the FMA pipe
+//   BCF_CE3_FMA_PLANES  same for three-plane elements
+#ifndef BCF_CE1_FMA_MOD
+#define BCF_CE1_FMA_MOD 3
+#endif
+#ifndef BCF_CE2_FMA_PLANES
+#define BCF_CE2_FMA_PLANES 1
+#endif
+#ifndef BCF_CE3_FMA_PLANES
+#define BCF_CE3_FMA_PLANES 0
+#endif
 
 // After the call element i <= element j in the lexicographic plane order.
 template <int NP>
@@ -36,18 +86,19 @@ __device__ __forceinline__ void ce(uint32_t (&v)[NP][32], const int i, const int
 {
     if constexpr (NP == 1) {
         const uint32_t a = v[0][i], b = v[0][j];
-        v[0][i] = min(a, b);
-        v[0][j] = max(a, b);
+        const uint32_t lo = min(a, b);
+        v[0][i] = lo;
+        const bool fma = BCF_CE1_FMA_MOD > 0 && (i % (BCF_CE1_FMA_MOD > 0 ? BCF_CE1_FMA_MOD : 1)) != 0;
+        v[0][j] = fma ? other_of(a, b, lo) : max(a, b);
     } else {
-        const uint64_t x = (static_cast<uint64_t>(v[0][i]) << 32) | v[1][i];
-        const uint64_t y = (static_cast<uint64_t>(v[0][j]) << 32) | v[1][j];
-        bool sw = x > y;
-        if constexpr (NP == 3) sw = sw || (x == y && v[2][i] > v[2][j]);
+        const bool sw = elem_gt<NP>(v, i, j);
 #pragma unroll
         for (int p = 0; p < NP; ++p) {
             const uint32_t a = v[p][i], b = v[p][j];
-            v[p][i] = sw ? b : a;
-            v[p][j] = sw ? a : b;
+            const uint32_t lo = sw ? b : a;
+            v[p][i] = lo;
+            constexpr int FMA_PLANES = (NP == 2) ? BCF_CE2_FMA_PLANES : BCF_CE3_FMA_PLANES;
+            v[p][j] = (p >= NP - FMA_PLANES) ? other_of(a, b, lo) : (sw ? a : b);
         }
     }
 }
