@@ -177,9 +177,11 @@ inline bool pipe_eligible(size_t run_len)
     return !forced_v1;
 }
 
-bcf_status launch_merge_pipe(const uint32_t *kin, uint32_t *kout, uint32_t *splits, size_t n, size_t run_len,
-                             cudaStream_t s)
+template <class E>
+bcf_status launch_merge_pipe(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits, size_t n,
+                             size_t run_len, cudaStream_t s)
 {
+    using C = pipe::Cfg<E>;
     const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
     if (shares == 0) return BCF_OK;
     static int num_sms = 0;
@@ -188,20 +190,22 @@ bcf_status launch_merge_pipe(const uint32_t *kin, uint32_t *kout, uint32_t *spli
         if (cudaGetDevice(&dev) != cudaSuccess ||
             cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
             return BCF_ERR_CUDA;
-        if (cudaFuncSetAttribute(pipe::merge_pipe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)pipe::SmemLayout::total) != cudaSuccess)
+        if (cudaFuncSetAttribute(pipe::merge_pipe_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)C::total) != cudaSuccess) {
+            num_sms = 0;
             return BCF_ERR_CUDA;
+        }
     }
     if (2 * run_len > (size_t)pipe::SH) {
         LaunchTimer t(BCF_KERNEL_PARTITION, s);
         const unsigned blocks = static_cast<unsigned>((shares + 1 + 127) / 128);
-        pipe::partition_share_kernel<<<blocks, 128, 0, s>>>(kin, splits, n, run_len, shares);
+        pipe::partition_share_kernel<E><<<blocks, 128, 0, s>>>(kin, vin, splits, n, run_len, shares);
     }
     {
         LaunchTimer t(BCF_KERNEL_MERGE, s);
-        const unsigned long long cap = 2ull * num_sms;
+        const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * num_sms;
         const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
-        pipe::merge_pipe_kernel<<<blocks, pipe::THREADS, pipe::SmemLayout::total, s>>>(kin, kout, splits, n, run_len, shares);
+        pipe::merge_pipe_kernel<E><<<blocks, pipe::THREADS, C::total, s>>>(kin, vin, kout, vout, splits, n, run_len, shares);
     }
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }
@@ -274,15 +278,13 @@ bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *
         void *kd = to_a ? ka : kb;
         uint32_t *vd = to_a ? va : vb;
         bcf_status st;
-        if constexpr (E::NP == 1) {
-            if (pipe_eligible(l)) {
-                st = launch_merge_pipe(static_cast<const uint32_t *>(ksrc), static_cast<uint32_t *>(kd), splits, n, l, s);
-                if (st != BCF_OK) return st;
-                ksrc = kd;
-                vsrc = vd;
-                to_a = !to_a;
-                continue;
-            }
+        if (pipe_eligible(l)) {
+            st = launch_merge_pipe<E>(ksrc, vsrc, kd, vd, splits, n, l, s);
+            if (st != BCF_OK) return st;
+            ksrc = kd;
+            vsrc = vd;
+            to_a = !to_a;
+            continue;
         }
         st = launch_partition<E>(ksrc, vsrc, splits, g, s);
         if (st != BCF_OK) return st;

@@ -1,5 +1,5 @@
-// bcf_merge_pipe.cuh -- the production merge round for power-of-two run lengths (rows a5-a9):
-// a persistent, warp-specialised kernel fed by TMA bulk copies.
+// bcf_merge_pipe.cuh -- the production merge round for power-of-two run lengths (rows a5-a9), every
+// element type: a persistent, warp-specialised kernel fed by TMA bulk copies.
 //
 // PAPER.md section 2 (L83-85): "we treat Theta(M) elements as a single contiguous block and transfer
 // these blocks between the global and shared memories"; section 3.2 (L127-129): merge pages in
@@ -21,6 +21,11 @@
 //                stage buffer straight into the column layout (word address consecutive across
 //                lanes: conflict-free for any offset), releases the stage, and runs SHEARSORT-MERGE
 //                (column merger, skewed transpose, row merger, coalesced 128-bit stores).
+//
+// Multi-plane elements ((u32,u32), u64, (u64,u32)): the stage buffer holds the SoA pieces as they
+// are in global memory (a key region of 4- or 8-byte keys, a value region), the search compares
+// (key, value) lexicographically, and the transposes go through ONE 4 KiB scratch plane per warp,
+// plane after plane, so that two stage buffers of 8192 twelve-byte elements still fit one SM.
 #pragma once
 #include <utility>
 
@@ -32,24 +37,32 @@ namespace pipe {
 constexpr int NW = 8;                    // consumer warps per CTA
 constexpr int SH = NW * TILE;            // outputs per share
 constexpr int NSTAGE = 2;
-constexpr int STAGE_WORDS = SH + 32;     // room for the two aligned supersets
 constexpr int THREADS = (NW + 1) * 32;
+constexpr int REGION_SLACK = 128;        // bytes: room for the 16-byte aligned supersets of two pieces
 
 struct ShareMeta {
     int cnt;         // outputs of this share (<= SH)
-    int a_off;       // word offset of the A piece in the stage buffer ("large" rounds)
-    int a_len;
-    int b_off;
+    int a_len;       // elements taken from run A / run B ("large" rounds)
     int b_len;
-    int pad[3];
+    int ka_off;      // element offset of the first A / B key inside the key region
+    int kb_off;
+    int va_off;      // same for the value region (its alignment slack differs from the keys')
+    int vb_off;
+    int pad;
 };
 
-struct SmemLayout {
-    static constexpr size_t stage_bytes = size_t(STAGE_WORDS) * 4;
-    static constexpr size_t planes_off = NSTAGE * stage_bytes;
-    static constexpr size_t meta_off = planes_off + size_t(NW) * TILE * 4;
+template <class E>
+struct Cfg {
+    static constexpr int KB = E::KEY_BYTES;
+    static constexpr size_t key_region = size_t(SH) * KB + REGION_SLACK;
+    static constexpr size_t val_region = E::HAS_VAL ? size_t(SH) * 4 + REGION_SLACK : 0;
+    static constexpr size_t stage_bytes = key_region + val_region;
+    static constexpr size_t scratch_off = NSTAGE * stage_bytes;
+    static constexpr size_t meta_off = scratch_off + size_t(NW) * TILE * 4;
     static constexpr size_t bar_off = meta_off + NSTAGE * sizeof(ShareMeta);
     static constexpr size_t total = bar_off + 2 * NSTAGE * 8;
+    // 227 KiB of shared memory per SM, 1 KiB per CTA reserved by the system
+    static constexpr int ctas_per_sm = (2 * (total + 1024) <= 227 * 1024) ? 2 : 1;
 };
 
 // ------------------------------------------------------------------ PTX wrappers (mbarrier, TMA)
@@ -93,19 +106,46 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 
 // ------------------------------------------------------------------ in-shared-memory split search
 //
-// Co-rank of diagonal d of (A = buf[sA .. sA+la), B = buf[sB .. sB+lb)): smallest i with
-// NOT(A[i] <= B[d-1-i]) (A-first ties).  32-ary search: lane j probes i = lo + j * step with `step`
-// ODD, so the 32 probe addresses sA + i (and sB + d - 1 - i) fall into 32 distinct banks -- the
-// search itself obeys the paper's rule.  3 rounds for a range of 8192.
-__device__ __forceinline__ int corank_smem(const uint32_t *buf, const int sA, const int la, const int sB, const int lb,
+// Co-rank of diagonal d of (A = la elements at ka_off / va_off, B = lb elements at kb_off / vb_off):
+// smallest i with NOT(A[i] <= B[d-1-i]) in the (key, value) order (A-first ties).  32-ary search:
+// lane j probes i = lo + j * step with `step` ODD, so the 32 probe addresses of a 4-byte array fall
+// into 32 distinct banks, and the 16 probes of each half-warp of an 8-byte array into 16 distinct
+// bank pairs -- the search itself obeys the paper's rule.  3 rounds for 8192.
+template <class E>
+__device__ __forceinline__ bool elem_le_smem(const unsigned char *kreg, const unsigned char *vreg, const int ia, const int ib,
+                                             const int va, const int vb)
+{
+    if constexpr (E::KEY_WORDS == 1) {
+        const uint32_t x = reinterpret_cast<const uint32_t *>(kreg)[ia], y = reinterpret_cast<const uint32_t *>(kreg)[ib];
+        if constexpr (E::HAS_VAL) {
+            const uint32_t p = reinterpret_cast<const uint32_t *>(vreg)[va], q = reinterpret_cast<const uint32_t *>(vreg)[vb];
+            return x < y || (x == y && p <= q);
+        } else {
+            return x <= y;
+        }
+    } else {
+        const unsigned long long x = reinterpret_cast<const unsigned long long *>(kreg)[ia];
+        const unsigned long long y = reinterpret_cast<const unsigned long long *>(kreg)[ib];
+        if constexpr (E::HAS_VAL) {
+            const uint32_t p = reinterpret_cast<const uint32_t *>(vreg)[va], q = reinterpret_cast<const uint32_t *>(vreg)[vb];
+            return x < y || (x == y && p <= q);
+        } else {
+            return x <= y;
+        }
+    }
+}
+
+template <class E>
+__device__ __forceinline__ int corank_smem(const unsigned char *kreg, const unsigned char *vreg, const ShareMeta &m,
                                            const int d, const int lane)
 {
-    int lo = max(0, d - lb), hi = min(d, la);
+    int lo = max(0, d - m.b_len), hi = min(d, m.a_len);
     while (lo < hi) {
         const int step = (((hi - lo) + 31) >> 5) | 1;
         const int mid = lo + lane * step;
         bool le = false;
-        if (mid < hi) le = buf[sA + mid] <= buf[sB + d - 1 - mid];
+        if (mid < hi)
+            le = elem_le_smem<E>(kreg, vreg, m.ka_off + mid, m.kb_off + d - 1 - mid, m.va_off + mid, m.vb_off + d - 1 - mid);
         const int c = __popc(__ballot_sync(0xFFFFFFFFu, le));
         const int nlo = c ? lo + (c - 1) * step + 1 : lo;
         hi = min(hi, lo + c * step);
@@ -118,9 +158,10 @@ __device__ __forceinline__ int corank_smem(const uint32_t *buf, const int sA, co
 //
 // One thread per share boundary s in [0, num_shares]: co-rank of output diagonal SH * s inside its
 // pair (clamped to the pair's length).  Only launched for rounds with 2 L > SH.
+template <class E>
 __global__ void __launch_bounds__(128)
-partition_share_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ splits, const unsigned long long n,
-                       const unsigned long long L, const unsigned long long num_shares)
+partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
+                       const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)
 {
     const unsigned long long s = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (s > num_shares) return;
@@ -135,15 +176,19 @@ partition_share_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ 
     unsigned long long hi = min(d, alen);
     while (lo < hi) {
         const unsigned long long mid = (lo + hi) >> 1;
-        if (__ldg(kin + a0 + mid) <= __ldg(kin + b0 + (d - 1 - mid))) lo = mid + 1;
+        if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
         else hi = mid;
     }
     splits[s] = static_cast<uint32_t>(lo);
 }
 
-// Register slot K of the column layout: two predicated shared loads with immediate offsets.
+// ------------------------------------------------------------------ stage buffer -> column registers
+//
+// Register slot K of the column layout (position p = 32 K + lane of the bitonic sequence
+// A' || max-padding || reverse(B')): two predicated shared loads with immediate offsets per array.
+// Within each load the active lanes read consecutive elements: conflict-free for any offset.
 template <int K>
-__device__ __forceinline__ uint32_t load_column_slot(const int xa, const int xb, const uint32_t addrA, const uint32_t addrB)
+__device__ __forceinline__ uint32_t load_slot32(const int xa, const int xb, const uint32_t addrA, const uint32_t addrB)
 {
     uint32_t r = SENTINEL;
     asm volatile(
@@ -159,25 +204,131 @@ __device__ __forceinline__ uint32_t load_column_slot(const int xa, const int xb,
     return r;
 }
 
-template <int... Ks>
-__device__ __forceinline__ void load_columns(uint32_t (&v)[32], const int xa, const int xb, const uint32_t addrA,
-                                             const uint32_t addrB, std::integer_sequence<int, Ks...>)
+template <int K>
+__device__ __forceinline__ void load_slot64(uint32_t &hi, uint32_t &lo, const int xa, const int xb, const uint32_t addrA,
+                                            const uint32_t addrB)
 {
-    ((v[Ks] = load_column_slot<Ks>(xa, xb, addrA, addrB)), ...);
+    hi = SENTINEL;
+    lo = SENTINEL;
+    asm volatile(
+        "{\n"
+        ".reg .pred pa, pb;\n"
+        "setp.gt.s32 pa, %2, %4;\n"
+        "setp.ge.s32 pb, %3, %5;\n"
+        "@pa ld.shared.v2.u32 {%0, %1}, [%6+%8];\n"
+        "@pb ld.shared.v2.u32 {%0, %1}, [%7+%9];\n"
+        "}\n"
+        : "+r"(lo), "+r"(hi)
+        : "r"(xa), "r"(xb), "n"(32 * K), "n"(-32 * K), "r"(addrA), "r"(addrB), "n"(256 * K), "n"(-256 * K));
+}
+
+template <class E, int... Ks>
+__device__ __forceinline__ void load_columns(uint32_t (&v)[E::NP][32], const int xa, const int xb, const uint32_t kA,
+                                             const uint32_t kB, const uint32_t vA, const uint32_t vB,
+                                             std::integer_sequence<int, Ks...>)
+{
+    if constexpr (E::KEY_WORDS == 1) ((v[0][Ks] = load_slot32<Ks>(xa, xb, kA, kB)), ...);
+    else (load_slot64<Ks>(v[0][Ks], v[1][Ks], xa, xb, kA, kB), ...);
+    if constexpr (E::HAS_VAL) ((v[E::KEY_WORDS][Ks] = load_slot32<Ks>(xa, xb, vA, vB)), ...);
+}
+
+// ------------------------------------------------------------------ rows -> global through one scratch plane
+//
+// store_rows (bcf_kernels.cuh) with a single 4 KiB scratch plane per warp: the planes of the
+// element go through it one after the other.  Same access patterns, same conflict-freedom.
+template <class E>
+__device__ __forceinline__ void store_rows_seq(uint32_t *scratch, void *keys, uint32_t *vals, const size_t base,
+                                               const int cnt, const bool full, const int lane, uint32_t (&v)[E::NP][32])
+{
+    if (full) {
+        if constexpr (E::KEY_WORDS == 1) {
+            row_store(scratch, v[0], lane);
+            __syncwarp();
+            uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint32_t *>(keys) + base);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
+                stg128(pk + 32 * m + lane, *reinterpret_cast<const uint4 *>(scratch + w));
+            }
+        } else {
+            row_store(scratch, v[0], lane);
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {     // this lane's high words of keys 64 m + 2 lane, + 1
+                const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
+                const uint2 h = *reinterpret_cast<const uint2 *>(scratch + w);
+                v[0][2 * m] = h.x; v[0][2 * m + 1] = h.y;
+            }
+            __syncwarp();
+            row_store(scratch, v[1], lane);
+            __syncwarp();
+            uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint64_t *>(keys) + base);
+#pragma unroll
+            for (int m = 0; m < 16; ++m) {
+                const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
+                const uint2 l = *reinterpret_cast<const uint2 *>(scratch + w);
+                stg128(pk + 32 * m + lane, make_uint4(l.x, v[0][2 * m], l.y, v[0][2 * m + 1]));
+            }
+        }
+        if constexpr (E::HAS_VAL) {
+            __syncwarp();
+            row_store(scratch, v[E::KEY_WORDS], lane);
+            __syncwarp();
+            uint4 *pv = reinterpret_cast<uint4 *>(vals + base);
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const int w = chunk_word(4 * m + (lane >> 3), lane & 7);
+                stg128(pv + 32 * m + lane, *reinterpret_cast<const uint4 *>(scratch + w));
+            }
+        }
+    } else {
+        // ragged end of the array: back to the column layout (position 32 k + lane), guarded stores
+#pragma unroll
+        for (int p = 0; p < E::NP; ++p) {
+            row_store(scratch, v[p], lane);
+            __syncwarp();
+            col_load<false>(scratch, v[p], lane);
+            __syncwarp();
+        }
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            if (32 * k + lane < cnt) {
+                const size_t g = base + 32 * k + lane;
+                if constexpr (E::KEY_WORDS == 1) stg32(static_cast<uint32_t *>(keys) + g, v[0][k]);
+                else stg64(reinterpret_cast<uint2 *>(keys) + g, make_uint2(v[1][k], v[0][k]));
+                if constexpr (E::HAS_VAL) stg32(vals + g, v[E::KEY_WORDS][k]);
+            }
+        }
+    }
+    __syncwarp();   // the scratch plane is reused by the warp's next sub-tile
 }
 
 // ------------------------------------------------------------------ the merge round
 
-__global__ void __launch_bounds__(THREADS, 2)
-merge_pipe_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ kout, const uint32_t *__restrict__ splits,
-                  const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)
+// 16-byte aligned superset [s, e) of elements [g, g + len) of an array of EB-byte elements.
+template <int EB>
+__device__ __forceinline__ void aligned_superset(const unsigned long long g, const int len, unsigned long long &s,
+                                                 unsigned long long &e)
 {
+    constexpr unsigned long long M = 16 / EB - 1;
+    s = g & ~M;
+    e = (g + len + M) & ~M;
+}
+
+template <class E>
+__global__ void __launch_bounds__(THREADS, Cfg<E>::ctas_per_sm)
+merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vin, void *__restrict__ kout,
+                  uint32_t *__restrict__ vout, const uint32_t *__restrict__ splits, const unsigned long long n,
+                  const unsigned long long L, const unsigned long long num_shares)
+{
+    using C = Cfg<E>;
+    constexpr int KB = C::KB;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint32_t *stage_buf = reinterpret_cast<uint32_t *>(smem_raw);
-    uint32_t *planes_all = reinterpret_cast<uint32_t *>(smem_raw + SmemLayout::planes_off);
-    ShareMeta *meta = reinterpret_cast<ShareMeta *>(smem_raw + SmemLayout::meta_off);
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + SmemLayout::bar_off);
+    uint32_t *scratch_all = reinterpret_cast<uint32_t *>(smem_raw + C::scratch_off);
+    ShareMeta *meta = reinterpret_cast<ShareMeta *>(smem_raw + C::meta_off);
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + C::bar_off);
     uint64_t *empty = full + NSTAGE;
+    const unsigned char *kin = static_cast<const unsigned char *>(kin_);
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -198,22 +349,28 @@ merge_pipe_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ kout,
         for (unsigned long long s = blockIdx.x; s < num_shares; s += gridDim.x, ++it) {
             const int st = it % NSTAGE;
             const uint32_t ph = (it / NSTAGE) & 1u;
-            uint32_t *buf = stage_buf + st * STAGE_WORDS;
+            unsigned char *kreg = smem_raw + st * C::stage_bytes;
+            unsigned char *vreg = kreg + C::key_region;
             mbar_wait(&empty[st], ph ^ 1u);
             const unsigned long long out0 = s * SH;
             const int cnt = static_cast<int>(min(static_cast<unsigned long long>(SH), n - out0));
             ShareMeta m;
             m.cnt = cnt;
+            m.pad = 0;
             if (small_round) {
-                m.a_off = 0; m.a_len = 0; m.b_off = 0; m.b_len = 0;
+                m.a_len = 0; m.b_len = 0; m.ka_off = 0; m.kb_off = 0; m.va_off = 0; m.vb_off = 0;
                 if ((cnt & 3) == 0) {
                     if (lane == 0) {
                         meta[st] = m;
-                        mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(cnt) * 4u);
-                        bulk_g2s(buf, kin + out0, static_cast<uint32_t>(cnt) * 4u, &full[st]);
+                        mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(cnt) * (KB + (E::HAS_VAL ? 4u : 0u)));
+                        bulk_g2s(kreg, kin + out0 * KB, static_cast<uint32_t>(cnt) * KB, &full[st]);
+                        if constexpr (E::HAS_VAL) bulk_g2s(vreg, vin + out0, static_cast<uint32_t>(cnt) * 4u, &full[st]);
                     }
                 } else {   // ragged end of the array: plain cooperative copy
-                    for (int i = lane; i < cnt; i += 32) buf[i] = kin[out0 + i];
+                    for (int i = lane; i < cnt * (KB / 4); i += 32)
+                        reinterpret_cast<uint32_t *>(kreg)[i] = reinterpret_cast<const uint32_t *>(kin + out0 * KB)[i];
+                    if constexpr (E::HAS_VAL)
+                        for (int i = lane; i < cnt; i += 32) reinterpret_cast<uint32_t *>(vreg)[i] = vin[out0 + i];
                     __syncwarp();
                     if (lane == 0) { meta[st] = m; mbar_arrive(&full[st]); }
                 }
@@ -227,25 +384,49 @@ merge_pipe_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ kout,
                 const unsigned long long I1 = (D1 >= alen + blen) ? alen : splits[s + 1];
                 const unsigned long long ga = a0 + I0, gb = b0 + (D0 - I0);
                 const int la = static_cast<int>(I1 - I0), lb = cnt - la;
-                const unsigned long long sa = ga & ~3ull, ea = (ga + la + 3) & ~3ull;
-                const unsigned long long sb = gb & ~3ull, eb = (gb + lb + 3) & ~3ull;
-                const int wordsA = la ? static_cast<int>(ea - sa) : 0;
-                const int wordsB = lb ? static_cast<int>(eb - sb) : 0;
-                m.a_off = static_cast<int>(ga - sa);
+                unsigned long long ksa, kea, ksb, keb, vsa = 0, vea = 0, vsb = 0, veb = 0;
+                aligned_superset<KB>(ga, la, ksa, kea);
+                aligned_superset<KB>(gb, lb, ksb, keb);
+                const int kA = la ? static_cast<int>(kea - ksa) : 0;
+                const int kB = lb ? static_cast<int>(keb - ksb) : 0;
                 m.a_len = la;
-                m.b_off = wordsA + static_cast<int>(gb - sb);
                 m.b_len = lb;
-                const bool bulk_ok = (!la || ea <= n) && (!lb || eb <= n);
+                m.ka_off = static_cast<int>(ga - ksa);
+                m.kb_off = kA + static_cast<int>(gb - ksb);
+                int vA = 0, vB = 0;
+                m.va_off = 0;
+                m.vb_off = 0;
+                bool bulk_ok = (!la || kea <= n) && (!lb || keb <= n);
+                if constexpr (E::HAS_VAL) {
+                    aligned_superset<4>(ga, la, vsa, vea);
+                    aligned_superset<4>(gb, lb, vsb, veb);
+                    vA = la ? static_cast<int>(vea - vsa) : 0;
+                    vB = lb ? static_cast<int>(veb - vsb) : 0;
+                    m.va_off = static_cast<int>(ga - vsa);
+                    m.vb_off = vA + static_cast<int>(gb - vsb);
+                    bulk_ok = bulk_ok && (!la || vea <= n) && (!lb || veb <= n);
+                }
                 if (bulk_ok) {
                     if (lane == 0) {
                         meta[st] = m;
-                        mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(wordsA + wordsB) * 4u);
-                        if (la) bulk_g2s(buf, kin + sa, static_cast<uint32_t>(wordsA) * 4u, &full[st]);
-                        if (lb) bulk_g2s(buf + wordsA, kin + sb, static_cast<uint32_t>(wordsB) * 4u, &full[st]);
+                        mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(kA + kB) * KB + static_cast<uint32_t>(vA + vB) * 4u);
+                        if (la) bulk_g2s(kreg, kin + ksa * KB, static_cast<uint32_t>(kA) * KB, &full[st]);
+                        if (lb) bulk_g2s(kreg + size_t(kA) * KB, kin + ksb * KB, static_cast<uint32_t>(kB) * KB, &full[st]);
+                        if constexpr (E::HAS_VAL) {
+                            if (la) bulk_g2s(vreg, vin + vsa, static_cast<uint32_t>(vA) * 4u, &full[st]);
+                            if (lb) bulk_g2s(vreg + size_t(vA) * 4, vin + vsb, static_cast<uint32_t>(vB) * 4u, &full[st]);
+                        }
                     }
                 } else {
-                    for (int i = lane; i < la; i += 32) buf[m.a_off + i] = kin[ga + i];
-                    for (int i = lane; i < lb; i += 32) buf[m.b_off + i] = kin[gb + i];
+                    uint32_t *kw = reinterpret_cast<uint32_t *>(kreg);
+                    const uint32_t *gk = reinterpret_cast<const uint32_t *>(kin);
+                    for (int i = lane; i < la * (KB / 4); i += 32) kw[m.ka_off * (KB / 4) + i] = gk[ga * (KB / 4) + i];
+                    for (int i = lane; i < lb * (KB / 4); i += 32) kw[m.kb_off * (KB / 4) + i] = gk[gb * (KB / 4) + i];
+                    if constexpr (E::HAS_VAL) {
+                        uint32_t *vw = reinterpret_cast<uint32_t *>(vreg);
+                        for (int i = lane; i < la; i += 32) vw[m.va_off + i] = vin[ga + i];
+                        for (int i = lane; i < lb; i += 32) vw[m.vb_off + i] = vin[gb + i];
+                    }
                     __syncwarp();
                     if (lane == 0) { meta[st] = m; mbar_arrive(&full[st]); }
                 }
@@ -255,54 +436,62 @@ merge_pipe_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ kout,
     }
 
     // ============================== consumer warps
-    uint32_t *planes = planes_all + warp * TILE;
+    uint32_t *scratch = scratch_all + warp * TILE;
     const int tile_off = warp * TILE;
     unsigned int it = 0;
     for (unsigned long long s = blockIdx.x; s < num_shares; s += gridDim.x, ++it) {
         const int st = it % NSTAGE;
         const uint32_t ph = (it / NSTAGE) & 1u;
-        const uint32_t *buf = stage_buf + st * STAGE_WORDS;
+        const unsigned char *kreg = smem_raw + st * C::stage_bytes;
+        const unsigned char *vreg = kreg + C::key_region;
         mbar_wait(&full[st], ph);
-        const ShareMeta m = meta[st];
+        ShareMeta m = meta[st];
         if (tile_off >= m.cnt) {            // ragged last share: nothing for this warp
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);
             continue;
         }
-        int sA, la, sB, lb, d0;
+        int d0;
         if (small_round) {
             const int l = static_cast<int>(L);
             const int pb = tile_off / (2 * l) * (2 * l);
-            la = min(l, m.cnt - pb);
-            lb = min(l, m.cnt - pb - la);
-            sA = pb; sB = pb + la; d0 = tile_off - pb;
+            m.a_len = min(l, m.cnt - pb);
+            m.b_len = min(l, m.cnt - pb - m.a_len);
+            m.ka_off = pb; m.kb_off = pb + m.a_len;
+            m.va_off = pb; m.vb_off = pb + m.a_len;
+            d0 = tile_off - pb;
         } else {
-            sA = m.a_off; la = m.a_len; sB = m.b_off; lb = m.b_len; d0 = tile_off;
+            d0 = tile_off;
         }
-        const int d1 = min(d0 + TILE, la + lb);
-        const int i0 = corank_smem(buf, sA, la, sB, lb, d0, lane);
-        const int i1 = corank_smem(buf, sA, la, sB, lb, d1, lane);
+        const int d1 = min(d0 + TILE, m.a_len + m.b_len);
+        const int i0 = corank_smem<E>(kreg, vreg, m, d0, lane);
+        const int i1 = corank_smem<E>(kreg, vreg, m, d1, lane);
         const int a = i1 - i0;                   // elements of A in this sub-tile
         const int b = (d1 - d0) - a;             // elements of B
         // column layout straight from the stage buffer: position p = 32 k + lane is A'[p] for p < a,
         // B'[1023 - p] for p >= 1024 - b, the maximum element in between (partial sub-tiles only).
-        // Two predicated loads per k: within each the active lanes read consecutive words.
-        const uint32_t addrA = smem_u32(buf + sA + i0 + lane);
-        const uint32_t addrB = smem_u32(buf + sB + (d0 - i0) + (TILE - 1) - lane);
+        const uint32_t kA = smem_u32(kreg) + static_cast<uint32_t>(m.ka_off + i0 + lane) * KB;
+        const uint32_t kB = smem_u32(kreg) + static_cast<uint32_t>(m.kb_off + (d0 - i0) + (TILE - 1) - lane) * KB;
+        const uint32_t vA = smem_u32(vreg) + static_cast<uint32_t>(m.va_off + i0 + lane) * 4u;
+        const uint32_t vB = smem_u32(vreg) + static_cast<uint32_t>(m.vb_off + (d0 - i0) + (TILE - 1) - lane) * 4u;
         const int xa = a - lane;                 // p < a        <=>  32 k < xa
-        const int xb = lane - (TILE - b);        // p >= 1024-b  <=>  32 k >= -xb  <=>  32 k + xb >= 0
-        uint32_t v[1][32];
-        load_columns(v[0], xa, xb, addrA, addrB, std::make_integer_sequence<int, 32>{});
+        const int xb = lane - (TILE - b);        // p >= 1024-b  <=>  32 k + xb >= 0
+        uint32_t v[E::NP][32];
+        load_columns<E>(v, xa, xb, kA, kB, vA, vB, std::make_integer_sequence<int, 32>{});
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);  // stage buffer may be refilled
 
-        line_bitonic_merge<1>(v);                // column pass
-        col_store<false>(planes, v[0], lane);
-        __syncwarp();
-        row_load(planes, v[0], lane);
-        line_bitonic_merge<1>(v);                // row pass
+        line_bitonic_merge<E::NP>(v);            // column pass
+#pragma unroll
+        for (int p = 0; p < E::NP; ++p) {
+            if (p) __syncwarp();
+            col_store<false>(scratch, v[p], lane);
+            __syncwarp();
+            row_load(scratch, v[p], lane);
+        }
+        line_bitonic_merge<E::NP>(v);            // row pass
         const int cnt = d1 - d0;
-        store_rows<Elem<1, false>>(planes, kout, nullptr, s * SH + tile_off, cnt, cnt == TILE, lane, v);
+        store_rows_seq<E>(scratch, kout, vout, s * SH + tile_off, cnt, cnt == TILE, lane, v);
     }
 }
 
