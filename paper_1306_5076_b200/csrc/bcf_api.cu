@@ -177,6 +177,17 @@ inline bool pipe_eligible(size_t run_len)
     return !forced_v1;
 }
 
+// Largest boundary count that takes the 32-lanes-per-boundary search (BCF_PART_WARP_MAX overrides).
+inline unsigned long long pipe_warp_search_max()
+{
+    static long long v = -1;
+    if (v < 0) {
+        const char *e = std::getenv("BCF_PART_WARP_MAX");
+        v = e ? std::atoll(e) : 4096;
+    }
+    return static_cast<unsigned long long>(v);
+}
+
 template <class E>
 bcf_status launch_merge_pipe(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits, size_t n,
                              size_t run_len, cudaStream_t s)
@@ -198,8 +209,14 @@ bcf_status launch_merge_pipe(const void *kin, const uint32_t *vin, void *kout, u
     }
     if (2 * run_len > (size_t)pipe::SH) {
         LaunchTimer t(BCF_KERNEL_PARTITION, s);
-        const unsigned blocks = static_cast<unsigned>((shares + 1 + 127) / 128);
-        pipe::partition_share_kernel<E><<<blocks, 128, 0, s>>>(kin, vin, splits, n, run_len, shares);
+        // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
+        if (shares + 1 <= pipe_warp_search_max()) {
+            const unsigned blocks = static_cast<unsigned>(((shares + 1) * 32 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
+            pipe::partition_share_kernel<E, 32><<<blocks, pipe::PART_THREADS, 0, s>>>(kin, vin, splits, n, run_len, shares);
+        } else {
+            const unsigned blocks = static_cast<unsigned>((shares + 1 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
+            pipe::partition_share_kernel<E, 1><<<blocks, pipe::PART_THREADS, 0, s>>>(kin, vin, splits, n, run_len, shares);
+        }
     }
     {
         LaunchTimer t(BCF_KERNEL_MERGE, s);

@@ -156,30 +156,51 @@ __device__ __forceinline__ int corank_smem(const unsigned char *kreg, const unsi
 
 // ------------------------------------------------------------------ a5 for shares: global split points
 //
-// One thread per share boundary s in [0, num_shares]: co-rank of output diagonal SH * s inside its
-// pair (clamped to the pair's length).  Only launched for rounds with 2 L > SH.
-template <class E>
-__global__ void __launch_bounds__(128)
+// G lanes per share boundary s in [0, num_shares]: co-rank of output diagonal SH * s inside its
+// pair (clamped to the pair's length) by a G-ary search -- lane j of the group probes
+// i = lo + j * step and one ballot narrows the range G-fold.  G = 32 needs 6 dependent rounds of
+// global loads for a pair of 2^27-element runs instead of 27 and wins while the launch is
+// latency-bound (few boundaries); with many boundaries the 64 probes per round make it
+// bandwidth-bound and the plain binary search (G = 1) is faster (measured).
+// Only launched for rounds with 2 L > SH.
+constexpr int PART_THREADS = 128;
+template <class E, int G>
+__global__ void __launch_bounds__(PART_THREADS)
 partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
                        const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)
 {
-    const unsigned long long s = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    const int j = threadIdx.x % G;                       // lane inside the group
+    const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
+    const unsigned long long s = (static_cast<unsigned long long>(blockIdx.x) * PART_THREADS + threadIdx.x) / G;
     if (s > num_shares) return;
     const unsigned long long out0 = s * SH;
     const unsigned long long a0 = out0 / (2 * L) * (2 * L);
-    if (a0 >= n) { splits[s] = 0; return; }
+    if (a0 >= n) { if (j == 0) splits[s] = 0; return; }
     const unsigned long long alen = min(L, n - a0);
     const unsigned long long b0 = a0 + alen;
     const unsigned long long blen = min(L, n - b0);
     const unsigned long long d = min(out0 - a0, alen + blen);
     unsigned long long lo = d > blen ? d - blen : 0ull;
     unsigned long long hi = min(d, alen);
-    while (lo < hi) {
-        const unsigned long long mid = (lo + hi) >> 1;
-        if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
-        else hi = mid;
+    if constexpr (G == 1) {
+        while (lo < hi) {
+            const unsigned long long mid = (lo + hi) >> 1;
+            if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
+            else hi = mid;
+        }
+    } else {
+        while (lo < hi) {
+            const unsigned long long step = (hi - lo + G - 1) / G;
+            const unsigned long long mid = lo + j * step;
+            bool le = false;
+            if (mid < hi) le = elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid));
+            const unsigned long long c = __popc(__ballot_sync(gmask, le) & gmask);
+            const unsigned long long nlo = c ? lo + (c - 1) * step + 1 : lo;
+            hi = min(hi, lo + c * step);
+            lo = nlo;
+        }
     }
-    splits[s] = static_cast<uint32_t>(lo);
+    if (j == 0) splits[s] = static_cast<uint32_t>(lo);
 }
 
 // ------------------------------------------------------------------ stage buffer -> column registers
