@@ -39,6 +39,7 @@ extern "C" {
 
 #define BCF_W 32            /* warp size = number of 4-byte shared memory banks */
 #define BCF_TILE 1024       /* M = w*w elements per tile / page           */
+#define BCF_SHARE 8192      /* outputs of a merge pass one CTA takes at a time (8 pages)              */
 
 /* A CUDA stream handle; identical to cudaStream_t / CUstream. */
 typedef struct CUstream_st *bcf_stream_t;
@@ -115,10 +116,45 @@ bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, siz
                                bcf_stream_t stream);
 
 /*
+ * bcf_merge_partition4 -- split-point search of one FOUR-RUN pass (two merge rounds of PAPER.md
+ * section 3, done on chip per read + write of the data).
+ * Runs 4g .. 4g+3 (run r = elements [r*run_len, min(n, (r+1)*run_len))) form group g; the pass
+ * output is cut into shares of BCF_SHARE elements.  For every share boundary
+ * s = 0 .. ceil(n / BCF_SHARE) at output position s * BCF_SHARE, inside the group that position
+ * falls into (4 run_len must be a multiple of BCF_SHARE):
+ *   d_splits[4 s + r] (uint32, device, 16-byte aligned) = number of elements of run r of the group
+ *   among the first d = s * BCF_SHARE - group_start outputs of the stable four-way merge (ties:
+ *   lower run first, then lower position), found by multi-sequence selection.
+ * A boundary at or past n receives the split of d clipped to the group's length (0 0 0 0 for a
+ * group that starts at or past n).  num_bounds must be ceil(n / BCF_SHARE) + 1.
+ */
+bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len,
+                                bcf_key_t kt, bcf_val_t vt, uint32_t *d_splits, size_t num_bounds,
+                                bcf_stream_t stream);
+
+/*
+ * Number of passes over global memory (one read + one write of all n elements each) that
+ * bcf_merge_runs takes from runs of run_len: a pass does two merge rounds where the four-run
+ * kernel applies (run_len = 1024 * 2^k and the element type's stage buffers fit one SM) and one
+ * round otherwise.  bcf_sort takes 1 + bcf_merge_pass_count(n, BCF_TILE, ..) passes.  Host only.
+ */
+int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt);
+
+/*
+ * Merge rounds per pass over global memory used by bcf_merge_runs / bcf_sort from now on
+ * (process-wide, host only): 1 = one round per read + write (Lemma 2), 2 = two rounds per
+ * read + write with the four-run kernel where it applies.  The result of every entry point is the
+ * same for both settings.  Anything else returns BCF_ERR_INVALID_ARG.
+ */
+bcf_status bcf_set_rounds_per_pass(int rounds);
+int bcf_get_rounds_per_pass(void);
+
+/*
  * bcf_merge_runs -- BCFMergesort's merging phase on already sorted runs.
- * PAPER.md section 3 (L103): ceil(log2(#runs)) rounds, each merging pairs of runs and each one
- * read + one write of all n elements (Lemma 2).  Every round is one partition
- * launch (above) and one merge launch in which a warp takes one share: it loads its piece of A
+ * PAPER.md section 3 (L103): ceil(log2(#runs)) rounds, each merging pairs of runs; the paper
+ * charges one read + one write of all n elements per round (Lemma 2), this library
+ * does two rounds per read + write where bcf_merge_pass_count says so.  Every pass is one
+ * partition launch (above) and one merge launch in which a warp takes one page at a time: it loads its piece of A
  * and its piece of B (together BCF_TILE elements, coalesced), merges them in shared
  * memory/registers with ONE ShearSort round -- SHEARSORT-MERGE, with the
  * second piece stored reversed so that one {column pass, row pass} is sufficient (reading A8) --
@@ -137,8 +173,8 @@ bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_
 /*
  * bcf_sort -- BCFMergesort (section 3, Appendix B): base case on
  * ceil(n / BCF_TILE) tiles (a last partial tile is padded with the maximum element on chip
- * only), then ceil(log2(ceil(n / BCF_TILE))) merge rounds ping-ponging between the data and the
- * workspace.  In place: the sorted result is in d_keys / d_vals for any n.
+ * only), then ceil(log2(ceil(n / BCF_TILE))) merge rounds in bcf_merge_pass_count(n, BCF_TILE, ..)
+ * passes ping-ponging between the data and the workspace.  In place: the sorted result is in d_keys / d_vals for any n.
  *   d_workspace : >= bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt) bytes.
  */
 bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt,

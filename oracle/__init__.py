@@ -149,3 +149,25 @@ def binary_merge_pagewise(ka, kb, va=None, vb=None, w=32):
     fn = getattr(_lib(), f"bcf_oracle_binary_merge_pagewise_{_suffix(a)}")
     _check(fn(_p(a), _p(av), a.size, _p(b), _p(bv), b.size, _p(ko), _p(vo), int(w)), "binary_merge_pagewise")
     return _ret(ko, vo)
+
+
+def corank_multi(runs_keys, d, runs_vals=None):
+    """Split of the first d outputs of the stable k-way merge of sorted runs (ties: lower run first,
+    then lower position) -- the definition the four-run partition of a pass must meet (the pass does
+    two rounds of PAPER.md:L103 at once; north_star: "split-point search so each CTA gets an equal
+    share of output").  Written out as the definition: concatenate the runs, sort STABLY by
+    (key, value) -- a stable sort of the concatenation orders equal elements by run, then position --
+    and count how many of the first d come from each run.  Returns a list of k counts summing to d."""
+    ks = [np.ascontiguousarray(r) for r in runs_keys]
+    lens = [r.size for r in ks]
+    if not 0 <= d <= sum(lens):
+        raise ValueError("d out of range")
+    cat = np.concatenate(ks) if ks else np.empty(0, dtype=np.uint32)
+    if runs_vals is None:
+        order = np.argsort(cat, kind="stable")
+    else:
+        vcat = np.concatenate([np.ascontiguousarray(v, dtype=np.uint32) for v in runs_vals])
+        order = np.lexsort((vcat, cat))      # lexsort is stable: last key is primary
+    first = order[:d]
+    bounds = np.cumsum([0] + lens)
+    return [int(np.count_nonzero((first >= bounds[r]) & (first < bounds[r + 1]))) for r in range(len(ks))]

@@ -19,6 +19,10 @@ from .binding import (  # noqa: F401
     layout_word,
     lib,
     merge_partition,
+    merge_partition4,
+    merge_pass_count,
+    get_rounds_per_pass,
+    set_rounds_per_pass,
     merge_runs,
     merge_runs_pagewise,
     num_shares,

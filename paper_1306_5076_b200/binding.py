@@ -13,6 +13,7 @@ BCF_VAL_NONE, BCF_VAL_U32 = 0, 1
 OP_SORT_TILES, OP_MERGE_RUNS, OP_SORT, OP_SORT_HOST, OP_MERGE_PAGEWISE = range(5)
 KERNEL_CLASSES = ("tile_sort", "partition", "merge", "merge_pagewise")
 TILE = 1024
+SHARE = 8192
 
 
 class BcfError(RuntimeError):
@@ -40,6 +41,9 @@ def lib():
     L.bcf_workspace_bytes.argtypes = [ci, sz, sz, ci, ci]
     L.bcf_sort_tiles.argtypes = [vp, vp, sz, ci, ci, vp]
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
+    L.bcf_set_rounds_per_pass.argtypes = [ci]
     L.bcf_merge_runs.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_runs_pagewise.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_sort.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
@@ -146,6 +150,35 @@ def merge_partition(keys, run_len, vals=None, stream=None):
     _check(lib().bcf_merge_partition(_dev(keys, "keys"), _dev(vals, "vals"), n, int(run_len), kt, vt,
                                      splits.data_ptr(), shares, _stream(stream)), "bcf_merge_partition")
     return splits[:shares]
+
+
+def merge_partition4(keys, run_len, vals=None, stream=None):
+    """bcf_merge_partition4: (ceil(n / 8192) + 1, 4) int32 tensor, row s = the four-run split of boundary s."""
+    torch = _torch()
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    bounds = -(-n // SHARE) + 1
+    splits = torch.empty((bounds, 4), dtype=torch.int32, device=keys.device)
+    _check(lib().bcf_merge_partition4(_dev(keys, "keys"), _dev(vals, "vals"), n, int(run_len), kt, vt,
+                                      splits.data_ptr(), bounds, _stream(stream)), "bcf_merge_partition4")
+    return splits
+
+
+def merge_pass_count(n, run_len, key_dtype=None, has_vals=False, kt=None, vt=None):
+    """bcf_merge_pass_count: passes over global memory bcf_merge_runs takes from runs of run_len."""
+    if kt is None:
+        kt = BCF_KEY_U64 if np.dtype(key_dtype).itemsize == 8 else BCF_KEY_U32
+        vt = BCF_VAL_U32 if has_vals else BCF_VAL_NONE
+    return int(lib().bcf_merge_pass_count(int(n), int(run_len), kt, vt))
+
+
+def set_rounds_per_pass(rounds):
+    """bcf_set_rounds_per_pass: 1 or 2 merge rounds per pass over global memory."""
+    _check(lib().bcf_set_rounds_per_pass(int(rounds)), "bcf_set_rounds_per_pass")
+
+
+def get_rounds_per_pass():
+    return int(lib().bcf_get_rounds_per_pass())
 
 
 def _merge(fn, name, op, keys, run_len, vals, out_keys, out_vals, workspace, stream):

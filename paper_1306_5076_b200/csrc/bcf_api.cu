@@ -9,6 +9,7 @@
 #include "bcf_kernels.cuh"
 #include "bcf_pagewise.cuh"
 #include "bcf_merge_pipe.cuh"
+#include "bcf_merge4.cuh"
 #include <cstdlib>
 
 using namespace bcf;
@@ -227,6 +228,81 @@ bcf_status launch_merge_pipe(const void *kin, const uint32_t *vin, void *kout, u
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }
 
+// Rounds per pass: 2 = the four-run kernel of bcf_merge4.cuh where it applies, 1 = one round per pass
+// everywhere.  Set by bcf_set_rounds_per_pass(); the initial value comes from BCF_MERGE_WAYS (2 or 4 runs
+// per pass) if set.
+#ifndef BCF_DEFAULT_ROUNDS_PER_PASS
+#define BCF_DEFAULT_ROUNDS_PER_PASS 1
+#endif
+int g_rounds_per_pass = -1;
+inline int rounds_per_pass()
+{
+    if (g_rounds_per_pass < 0) {
+        const char *e = std::getenv("BCF_MERGE_WAYS");
+        g_rounds_per_pass = e ? (std::atoi(e) == 4 ? 2 : 1) : BCF_DEFAULT_ROUNDS_PER_PASS;
+    }
+    return g_rounds_per_pass;
+}
+
+// Element types whose two stage buffers of a four-run share fit one SM (bcf_merge4.cuh).
+template <class E>
+inline bool merge4_eligible(size_t run_len)
+{
+    return pipe4::Cfg4<E>::fits && pipe_eligible(run_len) && rounds_per_pass() == 2;
+}
+
+template <class E>
+bcf_status launch_partition4(const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len,
+                             size_t num_bounds, cudaStream_t s)
+{
+    if (num_bounds == 0) return BCF_OK;
+    const unsigned blocks = static_cast<unsigned>((num_bounds + pipe4::PART4_THREADS - 1) / pipe4::PART4_THREADS);
+    {
+        LaunchTimer t(BCF_KERNEL_PARTITION, s);
+        pipe4::partition4_kernel<E><<<blocks, pipe4::PART4_THREADS, 0, s>>>(kin, vin, reinterpret_cast<uint4 *>(splits), n, run_len,
+                                                                           num_bounds, pipe4::SH);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+// One pass = two merge rounds: groups of four runs of run_len become one run of 4 run_len.
+template <class E>
+bcf_status launch_merge4(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits, size_t n,
+                         size_t run_len, cudaStream_t s)
+{
+    using C = pipe4::Cfg4<E>;
+    if constexpr (!C::fits) {
+        return BCF_ERR_INVALID_ARG;
+    } else {
+        const unsigned long long shares = (n + pipe4::SH - 1) / pipe4::SH;
+        if (shares == 0) return BCF_OK;
+        static int num_sms = 0;
+        if (!num_sms) {
+            int dev = 0;
+            if (cudaGetDevice(&dev) != cudaSuccess ||
+                cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+                return BCF_ERR_CUDA;
+            if (cudaFuncSetAttribute(pipe4::merge4_pipe_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)C::total) != cudaSuccess) {
+                num_sms = 0;
+                return BCF_ERR_CUDA;
+            }
+        }
+        if (4 * run_len > (size_t)pipe4::SH) {
+            const bcf_status st = launch_partition4<E>(kin, vin, splits, n, run_len, shares + 1, s);
+            if (st != BCF_OK) return st;
+        }
+        {
+            LaunchTimer t(BCF_KERNEL_MERGE, s);
+            const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * num_sms;
+            const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
+            pipe4::merge4_pipe_kernel<E><<<blocks, pipe4::THREADS, C::total, s>>>(
+                kin, vin, kout, vout, reinterpret_cast<const uint4 *>(splits), n, run_len, shares);
+        }
+        return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+    }
+}
+
 template <class E>
 bcf_status launch_pagewise(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, size_t run_len,
                            cudaStream_t s)
@@ -275,14 +351,37 @@ Workspace carve(void *base, size_t n, bcf_key_t kt, bcf_val_t vt, bool with_data
     w.vals = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
     if (with_data && vt == BCF_VAL_U32) off += align_up(n * 4, 256);
     w.splits = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
-    off += align_up((shares + 1) * 4, 256);
+    off += align_up((shares + 1) * 4 + 64, 256);   // + room for the uint4 entries of a four-run pass
     w.bytes = off;
     return w;
 }
 
-// The merging phase: `rounds` rounds starting from sorted runs of run_len in
-// (k0, v0); round r writes to dst[r].  Each round = partition + merge, one read + one write of
-// all n elements (Lemma 2).
+// The passes of the merging phase from sorted runs of run_len: ways[i] = 2 is one merge
+// round per read + write of the data (Lemma 2), ways[i] = 4 two rounds per read + write
+// (bcf_merge4.cuh).  An odd number of remaining rounds is made even by a two-way pass first.
+constexpr int MAX_PASSES = 40;
+template <class E>
+int plan_passes(size_t n, size_t run_len, int *ways)
+{
+    int np = 0;
+    for (size_t l = run_len; l < n && np < MAX_PASSES; ++np) {
+        const int remaining = ceil_log2((n + l - 1) / l);
+        const bool four = remaining % 2 == 0 && merge4_eligible<E>(l);
+        ways[np] = four ? 4 : 2;
+        l *= four ? 4 : 2;
+    }
+    return np;
+}
+
+int count_passes(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
+{
+    int ways[MAX_PASSES];
+    int np = 0;
+    BCF_DISPATCH(kt, vt, np = plan_passes<E>(n, run_len, ways));
+    return np;
+}
+
+// Pass i writes to dst[i]; each pass is one read + one write of all n elements.
 template <class E>
 bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
                         bool first_to_a, size_t n, size_t run_len, uint32_t *splits, cudaStream_t s)
@@ -290,26 +389,28 @@ bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *
     const void *ksrc = k0;
     const uint32_t *vsrc = v0;
     bool to_a = first_to_a;
-    for (size_t l = run_len; l < n; l *= 2) {
-        const PassGeom g = pass_geom(n, l);
+    int ways[MAX_PASSES];
+    const int np = plan_passes<E>(n, run_len, ways);
+    size_t l = run_len;
+    for (int i = 0; i < np; ++i) {
         void *kd = to_a ? ka : kb;
         uint32_t *vd = to_a ? va : vb;
         bcf_status st;
-        if (pipe_eligible(l)) {
+        if (ways[i] == 4) {
+            st = launch_merge4<E>(ksrc, vsrc, kd, vd, splits, n, l, s);
+        } else if (pipe_eligible(l)) {
             st = launch_merge_pipe<E>(ksrc, vsrc, kd, vd, splits, n, l, s);
+        } else {
+            const PassGeom g = pass_geom(n, l);
+            st = launch_partition<E>(ksrc, vsrc, splits, g, s);
             if (st != BCF_OK) return st;
-            ksrc = kd;
-            vsrc = vd;
-            to_a = !to_a;
-            continue;
+            st = launch_merge<E>(ksrc, vsrc, kd, vd, splits, g, s);
         }
-        st = launch_partition<E>(ksrc, vsrc, splits, g, s);
-        if (st != BCF_OK) return st;
-        st = launch_merge<E>(ksrc, vsrc, kd, vd, splits, g, s);
         if (st != BCF_OK) return st;
         ksrc = kd;
         vsrc = vd;
         to_a = !to_a;
+        l *= ways[i];
     }
     return BCF_OK;
 }
@@ -365,9 +466,10 @@ bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d
         if (vb && cudaMemcpyAsync(d_vals_out, d_vals_in, vb, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BCF_ERR_CUDA;
         return BCF_OK;
     }
-    const Workspace w = carve(d_workspace, n, kt, vt, rounds >= 2, pagewise ? 0 : max_shares(n, run_len));
-    // round r (1-based) writes to `out` when (rounds - r) is even, so the last round lands in out.
-    const bool first_to_out = ((rounds - 1) % 2 == 0);
+    // pass i (1-based) writes to `out` when (passes - i) is even, so the last pass lands in out.
+    const int passes = pagewise ? rounds : count_passes(n, run_len, kt, vt);
+    const Workspace w = carve(d_workspace, n, kt, vt, passes >= 2, pagewise ? 0 : max_shares(n, run_len));
+    const bool first_to_out = ((passes - 1) % 2 == 0);
     if (pagewise) {
         BCF_DISPATCH(kt, vt, st = pagewise_rounds<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
                                                      static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out,
@@ -411,7 +513,7 @@ size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_v
         if (run_len == 0) return 0;
         const int rounds = ceil_log2((n + run_len - 1) / run_len);
         if (rounds == 0) return 0;
-        return carve(nullptr, n, kt, vt, rounds >= 2, max_shares(n, run_len)).bytes;
+        return carve(nullptr, n, kt, vt, count_passes(n, run_len, kt, vt) >= 2, max_shares(n, run_len)).bytes;
     }
     case BCF_OP_MERGE_PAGEWISE: {
         if (run_len == 0) return 0;
@@ -460,6 +562,37 @@ bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, siz
     return st;
 }
 
+bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
+                                bcf_val_t vt, uint32_t *d_splits, size_t num_bounds, bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_splits || (vt == BCF_VAL_U32) != (d_vals_in != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_vals_in) || !aligned16(d_splits)) return BCF_ERR_MISALIGNED;
+    if (num_bounds != (n + BCF_SHARE - 1) / BCF_SHARE + 1) return BCF_ERR_INVALID_ARG;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    BCF_DISPATCH(kt, vt, st = launch_partition4<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, n, run_len,
+                                                   num_bounds, stream));
+    return st;
+}
+
+bcf_status bcf_set_rounds_per_pass(int rounds)
+{
+    if (rounds != 1 && rounds != 2) return BCF_ERR_INVALID_ARG;
+    g_rounds_per_pass = rounds;
+    return BCF_OK;
+}
+
+int bcf_get_rounds_per_pass(void) { return rounds_per_pass(); }
+
+int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
+{
+    if (!valid_types(kt, vt) || n == 0 || run_len == 0) return 0;
+    return count_passes(n, run_len, kt, vt);
+}
+
 bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out, size_t n,
                           size_t run_len, bcf_key_t kt, bcf_val_t vt, void *d_workspace, size_t workspace_bytes,
                           bcf_stream_t stream)
@@ -495,9 +628,9 @@ bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_
     const int rounds = ceil_log2(tiles);
     const Workspace w = carve(d_workspace, n, kt, vt, rounds > 0, rounds > 0 ? max_shares(n, TILE) : 0);
     uint32_t *vals = static_cast<uint32_t *>(d_vals);
-    // With an odd number of merge rounds the base case writes into the workspace, so that the
-    // last round lands in the caller's buffer without an extra copy.
-    const bool base_to_ws = (rounds % 2 == 1);
+    // With an odd number of merge passes the base case writes into the workspace, so that the
+    // last pass lands in the caller's buffer without an extra copy.
+    const bool base_to_ws = (count_passes(n, TILE, kt, vt) % 2 == 1);
     void *k0 = base_to_ws ? w.keys : d_keys;
     uint32_t *v0 = base_to_ws ? w.vals : vals;
     BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream));

@@ -20,6 +20,16 @@ def bcf():
     return m
 
 
+@pytest.fixture(params=[1, 2], ids=["1round", "2rounds"])
+def rpp(request, bcf):
+    """Both pass structures of the merging phase: one round per pass (Lemma 2) and two
+    rounds per pass (four-run kernel); the result must be the same unique sorted output."""
+    before = bcf.get_rounds_per_pass()
+    bcf.set_rounds_per_pass(request.param)
+    yield request.param
+    bcf.set_rounds_per_pass(before)
+
+
 def dev(a):
     """numpy unsigned array -> CUDA tensor holding the same bit pattern."""
     if a is None:
@@ -122,6 +132,34 @@ def test_merge_partition_matches_oracle_corank(bcf, kind, n, run_len):
         assert got == want, (j, got, want)
 
 
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("n,run_len,dup", [
+    (4 * 4096, 4096, False), (4 * 4096, 4096, True), (70001, 4096, True), (3 * 8192 + 5, 8192, False),
+    (100000, 16384, True), (8192 * 5 + 1, 8192, False), (1 << 17, 1 << 15, False), (9000, 4096, True),
+])
+def test_merge_partition4_matches_oracle_multiway_corank(bcf, kind, n, run_len, dup):
+    """Row a5 for four-run passes: every share boundary's split equals the definition (first d outputs
+    of the stable four-way merge), including short and missing runs in the last group."""
+    keys, vals = make(kind, n, seed=n + run_len, dup=dup)
+    if vals is None:
+        keys = workloads.sorted_runs(keys, run_len)
+    else:
+        keys, vals = workloads.sorted_runs(keys, run_len, vals)
+    got = bcf.merge_partition4(dev(keys), run_len, dev(vals)).cpu().numpy().view(np.uint32)
+    assert got.shape == (-(-n // 8192) + 1, 4)
+    for s in range(got.shape[0]):
+        out0 = s * 8192
+        g0 = out0 // (4 * run_len) * (4 * run_len)
+        if g0 >= n:
+            assert list(got[s]) == [0, 0, 0, 0]
+            continue
+        cuts = [min(n, g0 + r * run_len) for r in range(5)]
+        rk = [keys[cuts[r]:cuts[r + 1]] for r in range(4)]
+        rv = None if vals is None else [vals[cuts[r]:cuts[r + 1]] for r in range(4)]
+        d = min(out0 - g0, cuts[4] - g0)
+        assert list(got[s]) == oracle.corank_multi(rk, d, rv), (s, d)
+
+
 # ---------------------------------------------------------------- bcf_merge_runs (a6, a8, a9)
 
 
@@ -129,8 +167,9 @@ def test_merge_partition_matches_oracle_corank(bcf, kind, n, run_len):
 @pytest.mark.parametrize("n,run_len", [
     (2048, 1024), (8192, 1024), (5000, 1024), (10000, 2048), (4097, 4096), (3000, 700),
     (1 << 16, 1 << 12), (70001, 333), (1024, 1), (777, 1000), (1, 1), (2, 1), (40000, 20000), (40001, 13),
+    (5 * 4096 + 7, 4096), (9 * 2048, 2048), (7 * 1024 + 1, 1024), (1 << 18, 1 << 13), (300001, 1024), (3 * 32768 - 5, 32768),
 ])
-def test_merge_runs_matches_oracle(bcf, kind, n, run_len):
+def test_merge_runs_matches_oracle(bcf, kind, n, run_len, rpp):
     keys, vals = make(kind, n, seed=3 * n + run_len, dup=(n % 2 == 1))
     if vals is None:
         keys = workloads.sorted_runs(keys, run_len)
@@ -147,7 +186,7 @@ def test_merge_runs_matches_oracle(bcf, kind, n, run_len):
 
 
 @pytest.mark.parametrize("k", [2, 64, 1024])
-def test_merge_runs_config5b_shape(bcf, k):
+def test_merge_runs_config5b_shape(bcf, k, rpp):
     keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=1 << 18)
     out = bcf.merge_runs(dev(keys), run_len)
     assert np.array_equal(host(out, keys), oracle.merge_runs(keys, run_len))
@@ -186,8 +225,9 @@ def test_merge_runs_pagewise_matches_oracle(bcf, kind, n, run_len):
 
 
 @pytest.mark.parametrize("kind", KINDS)
-@pytest.mark.parametrize("n", [1, 2, 31, 1023, 1024, 1025, 2048, 5000, 3 * 1024 + 17, (1 << 16) + 17, 1 << 17])
-def test_sort_matches_oracle(bcf, kind, n):
+@pytest.mark.parametrize("n", [1, 2, 31, 1023, 1024, 1025, 2048, 5000, 3 * 1024 + 17, (1 << 16) + 17, 1 << 17,
+                               4096, 4097, 8192, 8193, 16 * 1024 + 3, 40 * 1024, (1 << 18) + 4099, 600001])
+def test_sort_matches_oracle(bcf, kind, n, rpp):
     keys, vals = make(kind, n, seed=n, dup=(n % 3 == 0))
     dk, dv = dev(keys), dev(vals)
     bcf.sort(dk, dv)
@@ -196,14 +236,14 @@ def test_sort_matches_oracle(bcf, kind, n):
 
 
 @pytest.mark.parametrize("dist", workloads.CFG4_VARIANTS)
-def test_sort_config4_distributions(bcf, dist):
+def test_sort_config4_distributions(bcf, dist, rpp):
     keys = workloads.cfg4_sort_u32(dist, n=(1 << 18) + 1000)
     d = dev(keys)
     bcf.sort(d)
     assert np.array_equal(host(d, keys), oracle.sort_full(keys))
 
 
-def test_sort_config3_and_5a_shapes(bcf):
+def test_sort_config3_and_5a_shapes(bcf, rpp):
     keys = workloads.cfg3_sort_u32(n=1 << 19)
     d = dev(keys)
     bcf.sort(d)

@@ -319,3 +319,34 @@ def test_binary_merge_pagewise_key_value():
     ko, vo = oracle.binary_merge_pagewise(ka, kb, va, vb)
     o = np.lexsort((v, k))
     assert np.array_equal(ko, k[o]) and np.array_equal(vo, v[o])
+
+
+def _kway_merge_trace(runs, d):
+    """Brute force: repeatedly take the smallest head, lowest run index on ties; counts after d steps."""
+    pos = [0] * len(runs)
+    for _ in range(d):
+        best = None
+        for r, run in enumerate(runs):
+            if pos[r] < len(run) and (best is None or run[pos[r]] < runs[best][pos[best]]):
+                best = r
+        pos[best] += 1
+    return pos
+
+
+def test_corank_multi_equals_kway_merge_trace_and_two_way_corank():
+    rng = np.random.default_rng(77)
+    for trial in range(300):
+        k = int(rng.integers(1, 5))
+        hi = int(rng.choice([2, 3, 50, 1 << 32]))
+        runs = [np.sort(rng.integers(0, hi, size=int(rng.integers(0, 12)), dtype=np.uint64).astype(np.uint32))
+                for _ in range(k)]
+        total = sum(r.size for r in runs)
+        for d in range(total + 1):
+            got = oracle.corank_multi(runs, d)
+            assert got == _kway_merge_trace([list(map(int, r)) for r in runs], d)
+            if k == 2:
+                assert got[0] == oracle.corank(runs[0], runs[1], d)
+    # (key, value) order: equal keys are split by value before run index
+    ka = [np.array([5, 5], np.uint32), np.array([5, 5], np.uint32)]
+    va = [np.array([2, 9], np.uint32), np.array([1, 3], np.uint32)]
+    assert [oracle.corank_multi(ka, d, va) for d in range(5)] == [[0, 0], [0, 1], [1, 1], [1, 2], [2, 2]]
