@@ -286,7 +286,7 @@ __device__ __forceinline__ int load_page(const unsigned char *kreg, const unsign
     const int d0 = j * TILE;
     const int d1 = min(d0 + TILE, m.a_len + m.b_len);
     const int i0 = pipe::corank_smem<E>(kreg, vreg, m, d0, lane);
-    const int i1 = pipe::corank_smem<E>(kreg, vreg, m, d1, lane);
+    const int i1 = pipe::corank_smem<E>(kreg, vreg, m, d1, lane, i0, i0 + (d1 - d0));
     const int a = i1 - i0;
     const int b = (d1 - d0) - a;
     const uint32_t kA = pipe::smem_u32(kreg) + static_cast<uint32_t>(m.ka_off + i0 + lane) * KB;
@@ -512,9 +512,9 @@ merge4_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ v
             w1 = M.w[q1] + j1 * TILE;
         }
         const int w0 = M.w[0], wq1 = M.w[1], wq2 = M.w[2], wq3 = M.w[3];
+        if (q1 >= 0) merge_page<E>(scratch, lane, v);
         consumer_barrier();          // every level-1 read of the stage buffer is done
         if (q1 >= 0) {
-            merge_page<E>(scratch, lane, v);
             store_rows_to<E, true>(scratch, kreg, reinterpret_cast<uint32_t *>(vreg), static_cast<size_t>(w1), cnt1,
                                    cnt1 == TILE, lane, v);
         }

@@ -137,9 +137,10 @@ __device__ __forceinline__ bool elem_le_smem(const unsigned char *kreg, const un
 
 template <class E>
 __device__ __forceinline__ int corank_smem(const unsigned char *kreg, const unsigned char *vreg, const ShareMeta &m,
-                                           const int d, const int lane)
+                                           const int d, const int lane, const int lo_min = 0, const int hi_max = 1 << 30)
 {
-    int lo = max(0, d - m.b_len), hi = min(d, m.a_len);
+    // [lo_min, hi_max]: a range the caller already knows (the co-rank of an earlier diagonal bounds this one)
+    int lo = max(max(0, d - m.b_len), lo_min), hi = min(min(d, m.a_len), hi_max);
     while (lo < hi) {
         const int step = (((hi - lo) + 31) >> 5) | 1;
         const int mid = lo + lane * step;
@@ -486,7 +487,7 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
         }
         const int d1 = min(d0 + TILE, m.a_len + m.b_len);
         const int i0 = corank_smem<E>(kreg, vreg, m, d0, lane);
-        const int i1 = corank_smem<E>(kreg, vreg, m, d1, lane);
+        const int i1 = corank_smem<E>(kreg, vreg, m, d1, lane, i0, i0 + (d1 - d0));
         const int a = i1 - i0;                   // elements of A in this sub-tile
         const int b = (d1 - d0) - a;             // elements of B
         // column layout straight from the stage buffer: position p = 32 k + lane is A'[p] for p < a,
