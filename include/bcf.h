@@ -98,6 +98,27 @@ bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles,
                           bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
 
 /*
+ * bcf_sort_tiles_mergesort -- same contract and same (unique) result as bcf_sort_tiles with a
+ * cheaper network inside the same conflict-free framework: every row sorted once (Batcher), then
+ * for T = 1..5 every block of 2^T rows is formed from its two sorted halves by ONE round
+ * {column pass, row pass} of the paper's page merge (SHEARSORT-MERGE, with the
+ * second half read reversed, reading A8), so all later line operations are bitonic mergers:
+ * 831 comparators per thread instead of ShearSort's 2101, the same 10 sweeps through shared memory.
+ */
+bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles,
+                                    bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
+
+/*
+ * Base case bcf_sort uses from now on (process-wide, host only): BCF_BASE_SHEARSORT = the paper's
+ * tile ShearSort (bcf_sort_tiles), BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort.  The result
+ * of bcf_sort is the same for both.  Initial value: BCF_BASE_TILE_MERGESORT, or the integer in the
+ * environment variable BCF_BASE_CASE.
+ */
+typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1 } bcf_base_case;
+bcf_status bcf_set_base_case(int base);
+int bcf_get_base_case(void);
+
+/*
  * bcf_merge_partition -- split-point search of ONE merge pass (hot-path row a5).
  * Not in the paper: it replaces the sampled bucket distribution of PAPER.md section 3.2
  * (L131-143, Alg. 7), which the paper needs because its page-wise merge is sequential per pair
@@ -210,7 +231,8 @@ typedef enum {
     BCF_KERNEL_PARTITION = 1,
     BCF_KERNEL_MERGE = 2,
     BCF_KERNEL_MERGE_PAGEWISE = 3,
-    BCF_KERNEL_CLASSES = 4
+    BCF_KERNEL_CLASSES = 4,          /* classes with timing / launch counters                           */
+    BCF_KERNEL_TILE_MERGESORT = 4    /* bcf_kernel_info only; timed and counted as BCF_KERNEL_TILE_SORT */
 } bcf_kernel_class;
 
 /*
@@ -248,7 +270,9 @@ typedef enum {
                                    `step` (0..7): row 4*step + lane/8, chunk lane%8               */
     BCF_ACCESS_OUT_LOAD64 = 6,  /* lane reads 8 bytes: row 2*step + lane/16, words 2*(lane%16)..+1  */
     BCF_ACCESS_OUT_LOAD32 = 7,  /* lane reads 1 word: row step, column lane                        */
-    BCF_ACCESS_PATTERNS = 8
+    BCF_ACCESS_COL_LOAD_LEVEL = 8, /* tile mergesort, step = 32 * (T - 1) + k for level T = 1..5, register k:
+                                   thread c reads position 32 k + c of P || reverse(Q) of its block of 2^T rows */
+    BCF_ACCESS_PATTERNS = 9
 } bcf_access_pattern;
 
 /*

@@ -31,6 +31,11 @@ from .binding import (  # noqa: F401
     sort,
     sort_host,
     sort_tiles,
+    sort_tiles_mergesort,
+    set_base_case,
+    get_base_case,
+    BASE_SHEARSORT,
+    BASE_TILE_MERGESORT,
     version,
     workspace_bytes,
 )

@@ -40,6 +40,8 @@ def lib():
     L.bcf_workspace_bytes.restype = sz
     L.bcf_workspace_bytes.argtypes = [ci, sz, sz, ci, ci]
     L.bcf_sort_tiles.argtypes = [vp, vp, sz, ci, ci, vp]
+    L.bcf_sort_tiles_mergesort.argtypes = [vp, vp, sz, ci, ci, vp]
+    L.bcf_set_base_case.argtypes = [ci]
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
@@ -138,6 +140,29 @@ def sort_tiles(keys, vals=None, stream=None):
     _check(lib().bcf_sort_tiles(_dev(keys, "keys"), _dev(vals, "vals"), n // TILE, kt, vt, _stream(stream)),
            "bcf_sort_tiles")
     return keys if vals is None else (keys, vals)
+
+
+def sort_tiles_mergesort(keys, vals=None, stream=None):
+    """bcf_sort_tiles_mergesort: same result as sort_tiles, merger network instead of ShearSort phases."""
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    if n % TILE:
+        raise ValueError("sort_tiles_mergesort needs a whole number of 1024-element tiles")
+    _check(lib().bcf_sort_tiles_mergesort(_dev(keys, "keys"), _dev(vals, "vals"), n // TILE, kt, vt, _stream(stream)),
+           "bcf_sort_tiles_mergesort")
+    return keys if vals is None else (keys, vals)
+
+
+BASE_SHEARSORT, BASE_TILE_MERGESORT = 0, 1
+
+
+def set_base_case(base):
+    """bcf_set_base_case: base case of sort(): BASE_SHEARSORT or BASE_TILE_MERGESORT."""
+    _check(lib().bcf_set_base_case(int(base)), "bcf_set_base_case")
+
+
+def get_base_case():
+    return int(lib().bcf_get_base_case())
 
 
 def merge_partition(keys, run_len, vals=None, stream=None):
@@ -252,7 +277,8 @@ def launch_counts():
 
 def kernel_info(kernel_class, kt=BCF_KEY_U32, vt=BCF_VAL_NONE):
     vals = [ctypes.c_int() for _ in range(5)]
-    _check(lib().bcf_kernel_info(KERNEL_CLASSES.index(kernel_class), kt, vt, *[ctypes.byref(v) for v in vals]),
+    cls = kernel_class if isinstance(kernel_class, int) else KERNEL_CLASSES.index(kernel_class)
+    _check(lib().bcf_kernel_info(cls, kt, vt, *[ctypes.byref(v) for v in vals]),
            "bcf_kernel_info")
     names = ("regs_per_thread", "smem_bytes_per_cta", "threads_per_cta", "ctas_per_sm", "local_bytes_per_thread")
     return dict(zip(names, (v.value for v in vals)))

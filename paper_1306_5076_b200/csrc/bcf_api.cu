@@ -111,23 +111,43 @@ struct LaunchTimer {
 template <class E>
 constexpr size_t warp_smem_bytes() { return size_t(E::NP) * TILE * 4; }
 
+// Base case of bcf_sort: BCF_BASE_SHEARSORT (the paper's tile sort) or BCF_BASE_TILE_MERGESORT (same
+// tile, same movement, mergers instead of full line sorts; bcf_kernels.cuh).  bcf_set_base_case().
+#ifndef BCF_DEFAULT_BASE_CASE
+#define BCF_DEFAULT_BASE_CASE BCF_BASE_TILE_MERGESORT
+#endif
+int g_base_case = -1;
+inline int base_case()
+{
+    if (g_base_case < 0) {
+        const char *e = std::getenv("BCF_BASE_CASE");
+        g_base_case = e ? (std::atoi(e) == BCF_BASE_SHEARSORT ? BCF_BASE_SHEARSORT : BCF_BASE_TILE_MERGESORT)
+                        : BCF_DEFAULT_BASE_CASE;
+    }
+    return g_base_case;
+}
+
 template <class E>
 bcf_status launch_tile_sort(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n,
-                            cudaStream_t s)
+                            cudaStream_t s, int algo = BCF_BASE_SHEARSORT)
 {
     const size_t tiles = (n + TILE - 1) / TILE;
     if (tiles == 0) return BCF_OK;
     const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(tile_sort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(tile_sort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+            cudaFuncSetAttribute(tile_mergesort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return BCF_ERR_CUDA;
         attr_set = true;
     }
     const size_t blocks = (tiles + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
     {
         LaunchTimer t(BCF_KERNEL_TILE_SORT, s);
-        tile_sort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
+        if (algo == BCF_BASE_TILE_MERGESORT)
+            tile_mergesort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
+        else
+            tile_sort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
     }
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }
@@ -532,7 +552,8 @@ size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_v
     return 0;
 }
 
-bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream)
+static bcf_status sort_tiles_common(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream,
+                                    int algo)
 {
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (num_tiles == 0) return BCF_OK;
@@ -542,9 +563,29 @@ bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_
     bcf_status st = check_device();
     if (st != BCF_OK) return st;
     BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, static_cast<uint32_t *>(d_vals), d_keys,
-                                                  static_cast<uint32_t *>(d_vals), num_tiles * TILE, stream));
+                                                  static_cast<uint32_t *>(d_vals), num_tiles * TILE, stream, algo));
     return st;
 }
+
+bcf_status bcf_sort_tiles(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream)
+{
+    return sort_tiles_common(d_keys, d_vals, num_tiles, kt, vt, stream, BCF_BASE_SHEARSORT);
+}
+
+bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt,
+                                    bcf_stream_t stream)
+{
+    return sort_tiles_common(d_keys, d_vals, num_tiles, kt, vt, stream, BCF_BASE_TILE_MERGESORT);
+}
+
+bcf_status bcf_set_base_case(int base)
+{
+    if (base != BCF_BASE_SHEARSORT && base != BCF_BASE_TILE_MERGESORT) return BCF_ERR_INVALID_ARG;
+    g_base_case = base;
+    return BCF_OK;
+}
+
+int bcf_get_base_case(void) { return base_case(); }
 
 bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
                                bcf_val_t vt, uint32_t *d_splits, size_t num_shares, bcf_stream_t stream)
@@ -633,7 +674,7 @@ bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_
     const bool base_to_ws = (count_passes(n, TILE, kt, vt) % 2 == 1);
     void *k0 = base_to_ws ? w.keys : d_keys;
     uint32_t *v0 = base_to_ws ? w.vals : vals;
-    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream));
+    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream, base_case()));
     if (st != BCF_OK || rounds == 0) return st;
     // round 1 writes to the buffer the base case did not write.
     BCF_DISPATCH(kt, vt, st = merge_rounds<E>(k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, TILE,
@@ -708,6 +749,7 @@ bcf_status bcf_kernel_info(int kernel_class, bcf_key_t kt, bcf_val_t vt, int *re
     BCF_DISPATCH(kt, vt, {
         switch (kernel_class) {
         case BCF_KERNEL_TILE_SORT: fn = (const void *)tile_sort_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
+        case BCF_KERNEL_TILE_MERGESORT: fn = (const void *)tile_mergesort_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
         case BCF_KERNEL_PARTITION: fn = (const void *)partition_kernel<E>; smem = 0; threads = 128; break;
         case BCF_KERNEL_MERGE: fn = (const void *)merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
         case BCF_KERNEL_MERGE_PAGEWISE: fn = (const void *)pagewise_merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
@@ -760,6 +802,12 @@ int bcf_layout_access(int pattern, int step, int lane, int *first_word)
         if (step > 7) return 0;
         *first_word = chunk_word(4 * step + (lane >> 3), lane & 7);
         return 4;
+    case BCF_ACCESS_COL_LOAD_LEVEL: {
+        if (step > 159) return 0;
+        const int T = step / 32 + 1, k = step % 32;
+        *first_word = elem_word(merge_level_row(T, k), merge_level_mirror(T, k) ? 31 - lane : lane);
+        return 1;
+    }
     case BCF_ACCESS_OUT_LOAD64:
         if (step > 15) return 0;
         *first_word = elem_word(2 * step + (lane >> 4), 2 * (lane & 15));

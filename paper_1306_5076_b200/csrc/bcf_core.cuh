@@ -157,6 +157,21 @@ __device__ __forceinline__ void line_bitonic_merge(uint32_t (&v)[NP][32])
     }
 }
 
+// Stages of stride 2^(T-1) .. 1 of a bitonic merger inside every block of 2^T consecutive registers
+// (T = 5 is line_bitonic_merge).  Used on column registers by the tile mergesort: a block of 2^T
+// rows of the page is a bitonic sequence of 32 * 2^T elements, and its stages of stride >= 32
+// elements are exactly these register stages of the thread that owns the column.
+template <int NP, int T>
+__device__ __forceinline__ void block_bitonic_merge(uint32_t (&v)[NP][32])
+{
+#pragma unroll
+    for (int s = (1 << (T - 1)); s >= 1; s >>= 1) {
+#pragma unroll
+        for (int k = 0; k < 32; ++k)
+            if ((k & s) == 0) ce<NP>(v, k, k + s);
+    }
+}
+
 // ------------------------------------------------------------------ shared-memory sweeps
 // `pl` points at one plane (1024 words) of the calling warp's tile.  All addresses are computed
 // from the lane; all register indices are constants.
@@ -196,6 +211,25 @@ __device__ __forceinline__ void col_store(uint32_t *pl, const uint32_t (&v)[32],
 {
 #pragma unroll
     for (int k = 0; k < 32; ++k) pl[elem_word(k, MIRROR ? mirrored_col(k, c) : c)] = v[k];
+}
+
+// Column sweep of the tile mergesort at level T: blocks of 2^T rows, each made of two sorted blocks
+// P (first half) and Q (second half) of 2^(T-1) rows.  The thread of column c reads, as register k,
+// position 32 k + c of the bitonic sequence P || reverse(Q): rows of P as they are, the rows of Q
+// in reverse order and mirrored (column 31 - c).  For a fixed k the 32 threads read the 32 words of
+// ONE row in a permuted order -> 32 distinct banks, like col_load.
+BCF_HD constexpr int merge_level_row(int T, int k)
+{
+    const int size = 1 << T, half = size >> 1, i = k & (size - 1);
+    return i < half ? k : (k - i) + half + (size - 1 - i);
+}
+BCF_HD constexpr bool merge_level_mirror(int T, int k) { return (k & ((1 << T) - 1)) >= (1 << (T - 1)); }
+
+template <int T>
+__device__ __forceinline__ void col_load_level(const uint32_t *pl, uint32_t (&v)[32], const int c)
+{
+#pragma unroll
+    for (int k = 0; k < 32; ++k) v[k] = pl[elem_word(merge_level_row(T, k), merge_level_mirror(T, k) ? 31 - c : c)];
 }
 
 }  // namespace bcf

@@ -271,6 +271,62 @@ tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vou
     }
 }
 
+// ------------------------------------------------------------------ tile mergesort (alternative base case)
+//
+// The same tile, the same conflict-free row <-> column movement, but the paper's own page merge
+// (SHEARSORT-MERGE, in the form of reading A8) applied inside the tile instead
+// of full ShearSort phases: rows are sorted once (Batcher, 191 comparators), then for T = 1..5 every
+// block of 2^T rows is formed from its two sorted halves by ONE round {column pass, row pass} --
+// the second half is read reversed, so every column of the block and then every row is bitonic and
+// the line "sorts" are mergers (16 T + 80 comparators per thread).  831 comparators per thread
+// instead of 2101, the same 10 sweeps through shared memory; the sorted tile is unique, so the
+// result is bit-identical to ShearSort's.  bcf_sort_tiles stays ShearSort (row a2); this kernel is
+// bcf_sort_tiles_mergesort and, by default, the base case of bcf_sort.
+template <class E, int T>
+__device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lane, uint32_t (&v)[E::NP][32])
+{
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) row_store(planes + p * TILE, v[p], lane);
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) col_load_level<T>(planes + p * TILE, v[p], lane);
+    block_bitonic_merge<E::NP, T>(v);                    // column pass: strides 2^(T-1) .. 1 rows
+    __syncwarp();                                        // mirrored reads: another thread's words are overwritten next
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
+    line_bitonic_merge<E::NP>(v);                        // row pass: strides 16 .. 1
+}
+
+template <class E>
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32)
+tile_mergesort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    uint32_t *planes = smem + warp * (E::NP * TILE);
+    const size_t num_tiles = (n + TILE - 1) / TILE;
+    const size_t stride = static_cast<size_t>(gridDim.x) * WARPS_PER_CTA;
+
+    for (size_t tile = static_cast<size_t>(blockIdx.x) * WARPS_PER_CTA + warp; tile < num_tiles; tile += stride) {
+        const size_t base = tile * TILE;
+        const int cnt = (n - base) < static_cast<size_t>(TILE) ? static_cast<int>(n - base) : TILE;
+        uint32_t v[E::NP][32];
+        if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
+        else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);
+        line_sort<E::NP>(v);                                // every row ascending
+        tile_merge_level<E, 1>(planes, lane, v);
+        tile_merge_level<E, 2>(planes, lane, v);
+        tile_merge_level<E, 3>(planes, lane, v);
+        tile_merge_level<E, 4>(planes, lane, v);
+        tile_merge_level<E, 5>(planes, lane, v);
+        store_rows<E>(planes, kout, vout, base, cnt, cnt == TILE, lane, v);
+    }
+}
+
 // ------------------------------------------------------------------ a5: merge partitioning
 
 struct PassGeom {

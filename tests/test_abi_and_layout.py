@@ -97,7 +97,7 @@ def test_layout_is_a_bijection_on_the_tile():
         assert {bcf.layout_word(r, c) // 32 for c in range(32)} == {r}
 
 
-STEPS = {0: 8, 1: 8, 2: 32, 3: 32, 4: 32, 5: 8, 6: 16, 7: 32}
+STEPS = {0: 8, 1: 8, 2: 32, 3: 32, 4: 32, 5: 8, 6: 16, 7: 32, 8: 160}
 
 
 @pytest.mark.parametrize("pattern", sorted(STEPS))
@@ -189,3 +189,20 @@ def test_paper_transpose_round_count():
     assert len(pairs) == w * w // 2 - w == 480
     missing = {(a, b) for a in range(w) for b in range(a + 1, w)} - pairs
     assert len(missing) == w // 2 and all(b - a == w // 2 for a, b in missing)
+
+
+def test_tile_mergesort_column_sweep_reads_P_then_reversed_Q():
+    """Pattern 8: at level T the thread of column c reads, as register k, position 32 k + c of the
+    sequence P || reverse(Q) of its block of 2^T rows (P, Q = the block's sorted halves, row-major).
+    Checked against that definition written out on a tile whose word at (r, c) holds 32 r + c."""
+    where = {bcf.layout_word(r, c): (r, c) for r in range(32) for c in range(32)}
+    for T in range(1, 6):
+        size, half = 1 << T, 1 << (T - 1)
+        for k in range(32):
+            base = k - k % size
+            P = [(base + i, c) for i in range(half) for c in range(32)]
+            Q = [(base + half + i, c) for i in range(half) for c in range(32)]
+            seq = P + Q[::-1]
+            for lane in range(32):
+                w, width = bcf.layout_access(8, 32 * (T - 1) + k, lane)
+                assert width == 1 and where[w] == seq[32 * (k - base) + lane]

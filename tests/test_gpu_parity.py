@@ -30,6 +30,15 @@ def rpp(request, bcf):
     bcf.set_rounds_per_pass(before)
 
 
+@pytest.fixture(params=[0, 1], ids=["shearsort", "tilemergesort"])
+def base(request, bcf):
+    """Both base cases of bcf_sort: the paper's tile ShearSort and the tile mergesort network."""
+    before = bcf.get_base_case()
+    bcf.set_base_case(request.param)
+    yield request.param
+    bcf.set_base_case(before)
+
+
 def dev(a):
     """numpy unsigned array -> CUDA tensor holding the same bit pattern."""
     if a is None:
@@ -96,6 +105,32 @@ def test_sort_tiles_types_and_counts(bcf, kind, tiles):
     bcf.sort_tiles(dk, dv)
     want = oracle.shearsort_tiles(keys, vals)
     assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("tiles", [1, 3, 4, 9, 130])
+def test_sort_tiles_mergesort_types_and_counts(bcf, kind, tiles):
+    """bcf_sort_tiles_mergesort: the same unique result as the ShearSort oracle on every element type."""
+    keys, vals = make(kind, tiles * 1024, seed=100 + tiles, dup=(tiles == 9))
+    if tiles >= 3:
+        keys[1024:2048] = keys[1024]                                    # all-equal tile
+        keys[2048:3072] = np.sort(keys[2048:3072])[::-1]                # reversed tile
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort_tiles_mergesort(dk, dv)
+    want = oracle.shearsort_tiles(keys, vals)
+    assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+def test_sort_tiles_mergesort_configs_1_and_2(bcf):
+    keys = workloads.cfg1_tiles_u32()
+    d = dev(keys)
+    bcf.sort_tiles_mergesort(d)
+    assert np.array_equal(host(d, keys), oracle.shearsort_tiles(keys))
+    keys, vals = workloads.cfg2_tiles_u32_u32(num_tiles=256)
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort_tiles_mergesort(dk, dv)
+    wk, wv = oracle.shearsort_tiles(keys, vals)
+    assert np.array_equal(host(dk, keys), wk) and np.array_equal(host(dv, vals), wv)
 
 
 def test_sort_tiles_config2_shape(bcf):
@@ -227,7 +262,7 @@ def test_merge_runs_pagewise_matches_oracle(bcf, kind, n, run_len):
 @pytest.mark.parametrize("kind", KINDS)
 @pytest.mark.parametrize("n", [1, 2, 31, 1023, 1024, 1025, 2048, 5000, 3 * 1024 + 17, (1 << 16) + 17, 1 << 17,
                                4096, 4097, 8192, 8193, 16 * 1024 + 3, 40 * 1024, (1 << 18) + 4099, 600001])
-def test_sort_matches_oracle(bcf, kind, n, rpp):
+def test_sort_matches_oracle(bcf, kind, n, rpp, base):
     keys, vals = make(kind, n, seed=n, dup=(n % 3 == 0))
     dk, dv = dev(keys), dev(vals)
     bcf.sort(dk, dv)
@@ -236,7 +271,7 @@ def test_sort_matches_oracle(bcf, kind, n, rpp):
 
 
 @pytest.mark.parametrize("dist", workloads.CFG4_VARIANTS)
-def test_sort_config4_distributions(bcf, dist, rpp):
+def test_sort_config4_distributions(bcf, dist, rpp, base):
     keys = workloads.cfg4_sort_u32(dist, n=(1 << 18) + 1000)
     d = dev(keys)
     bcf.sort(d)
@@ -293,7 +328,7 @@ def test_error_codes(bcf):
 
 
 def test_kernels_use_no_local_memory(bcf):
-    for cls in ("tile_sort", "partition", "merge"):
+    for cls in ("tile_sort", "partition", "merge", 4):   # 4 = BCF_KERNEL_TILE_MERGESORT
         for kt in (0, 1):
             for vt in (0, 1):
                 info = bcf.kernel_info(cls, kt, vt)
