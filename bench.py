@@ -34,6 +34,7 @@ sys.path.insert(0, ROOT)
 
 from paper_1306_5076_b200 import workloads  # noqa: E402
 
+TILE_ALGO = "shearsort"     # --tile-algo: network bcf_sort_tiles workloads (cfg1, cfg2) run
 METRIC = "sorted keys/sec"
 UNIT = "keys/s"
 
@@ -120,7 +121,7 @@ class Job:
         if self.op == "sort":
             b.sort(self.k, self.v, workspace=self.ws)
         elif self.op == "tiles":
-            b.sort_tiles(self.k, self.v)
+            (b.sort_tiles_mergesort if TILE_ALGO == "mergesort" else b.sort_tiles)(self.k, self.v)
         else:
             b.merge_runs(self.src_k, self.run_len, out_keys=self.out_k, workspace=self.ws)
 
@@ -328,6 +329,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4a", choices=sorted(WORKLOADS))
     ap.add_argument("--log2n", type=int, default=0, help="override the element count (debugging only)")
+    ap.add_argument("--base-case", default="tilemergesort", choices=["shearsort", "tilemergesort"],
+                    help="base case of bcf_sort: the paper's tile ShearSort or the tile mergesort network (default)")
+    ap.add_argument("--rounds-per-pass", type=int, default=1, choices=[1, 2],
+                    help="merge rounds per pass over global memory (2 = four-run kernel)")
+    ap.add_argument("--tile-algo", default="shearsort", choices=["shearsort", "mergesort"],
+                    help="network for the batch tile sort workloads cfg1 / cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-side", action="store_true", help="skip the short lines for the other configs")
@@ -355,6 +362,11 @@ def main():
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
+
+    global TILE_ALGO
+    TILE_ALGO = args.tile_algo
+    bcf.set_base_case(bcf.BASE_SHEARSORT if args.base_case == "shearsort" else bcf.BASE_TILE_MERGESORT)
+    bcf.set_rounds_per_pass(args.rounds_per_pass)
 
     desc, logn, gen, op, dtype = WORKLOADS[args.workload]
     n = 1 << (args.log2n or logn)
@@ -478,7 +490,9 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
             "config": {"workload": args.workload, "description": desc, "n": n, "bytes": eb * n,
-                       "passes": passes, "multi_gpu": "replicas only",
+                       "passes": passes, "base_case": args.base_case if op == "sort" else None,
+                       "tile_network": args.tile_algo if op == "tiles" else None,
+                       "merge_rounds_per_pass": args.rounds_per_pass, "multi_gpu": "replicas only",
                        "l2": "input and workspace (%d MiB each) %s the 126 MB L2; the input is restored from a "
                              "pristine copy before every step" % (eb * n >> 20, "exceed" if eb * n > 126e6 else "FIT IN"),
                        "timing": "CUDA events around each library call; restore copy outside the events",

@@ -81,14 +81,17 @@ __device__ __forceinline__ bool elem_gt(const uint32_t (&v)[NP][32], const int i
 #endif
 
 // After the call element i <= element j in the lexicographic plane order.
-template <int NP>
+// FMOD: keys-only comparator (i, j) forms its max on the FMA pipe when i % FMOD != 0 (0: never).  The
+// default suits the ALU-bound ShearSort and the merge kernels; the tile mergesort, which is bound by
+// issue slots and shared-memory latency instead, passes 0 (fewer instructions).
+template <int NP, int FMOD = BCF_CE1_FMA_MOD>
 __device__ __forceinline__ void ce(uint32_t (&v)[NP][32], const int i, const int j)
 {
     if constexpr (NP == 1) {
         const uint32_t a = v[0][i], b = v[0][j];
         const uint32_t lo = min(a, b);
         v[0][i] = lo;
-        const bool fma = BCF_CE1_FMA_MOD > 0 && (i % (BCF_CE1_FMA_MOD > 0 ? BCF_CE1_FMA_MOD : 1)) != 0;
+        const bool fma = FMOD > 0 && (i % (FMOD > 0 ? FMOD : 1)) != 0;
         v[0][j] = fma ? other_of(a, b, lo) : max(a, b);
     } else {
         const bool sw = elem_gt<NP>(v, i, j);
@@ -107,53 +110,53 @@ __device__ __forceinline__ void ce(uint32_t (&v)[NP][32], const int i, const int
 // PAPER.md:L111, L317 "BATCHERS-ODD-EVEN-MERGESORT(R)" on the 32 registers of one line
 // (191 compare-exchanges, depth 15).  Template recursion = full unrolling.
 
-template <int NP, int LO, int N, int R>
+template <int NP, int LO, int N, int R, int FMOD>
 struct OddEvenMerge {
     static __device__ __forceinline__ void run(uint32_t (&v)[NP][32])
     {
         constexpr int M = R * 2;
         if constexpr (M < N) {
-            OddEvenMerge<NP, LO, N, M>::run(v);
-            OddEvenMerge<NP, LO + R, N, M>::run(v);
+            OddEvenMerge<NP, LO, N, M, FMOD>::run(v);
+            OddEvenMerge<NP, LO + R, N, M, FMOD>::run(v);
 #pragma unroll
-            for (int i = LO + R; i + R < LO + N; i += M) ce<NP>(v, i, i + R);
+            for (int i = LO + R; i + R < LO + N; i += M) ce<NP, FMOD>(v, i, i + R);
         } else {
-            ce<NP>(v, LO, LO + R);
+            ce<NP, FMOD>(v, LO, LO + R);
         }
     }
 };
 
-template <int NP, int LO, int N>
+template <int NP, int LO, int N, int FMOD>
 struct OddEvenMergeSort {
     static __device__ __forceinline__ void run(uint32_t (&v)[NP][32])
     {
         if constexpr (N > 1) {
-            OddEvenMergeSort<NP, LO, N / 2>::run(v);
-            OddEvenMergeSort<NP, LO + N / 2, N / 2>::run(v);
-            OddEvenMerge<NP, LO, N, 1>::run(v);
+            OddEvenMergeSort<NP, LO, N / 2, FMOD>::run(v);
+            OddEvenMergeSort<NP, LO + N / 2, N / 2, FMOD>::run(v);
+            OddEvenMerge<NP, LO, N, 1, FMOD>::run(v);
         }
     }
 };
 
 // Sort the 32 elements of a line ascending.
-template <int NP>
+template <int NP, int FMOD = BCF_CE1_FMA_MOD>
 __device__ __forceinline__ void line_sort(uint32_t (&v)[NP][32])
 {
-    OddEvenMergeSort<NP, 0, 32>::run(v);
+    OddEvenMergeSort<NP, 0, 32, FMOD>::run(v);
 }
 
 // The last five stages (strides 16, 8, 4, 2, 1) of a bitonic merger applied to a line that is a
 // bitonic sequence: 80 compare-exchanges, depth 5.  Used by SHEARSORT-MERGE (reading A8): with
 // the second piece stored reversed every column and then every row of the page is bitonic, so
 // the line "sort" of PAPER.md:L129 needs only a merger.
-template <int NP>
+template <int NP, int FMOD = BCF_CE1_FMA_MOD>
 __device__ __forceinline__ void line_bitonic_merge(uint32_t (&v)[NP][32])
 {
 #pragma unroll
     for (int s = 16; s >= 1; s >>= 1) {
 #pragma unroll
         for (int k = 0; k < 32; ++k)
-            if ((k & s) == 0) ce<NP>(v, k, k + s);
+            if ((k & s) == 0) ce<NP, FMOD>(v, k, k + s);
     }
 }
 
@@ -161,14 +164,14 @@ __device__ __forceinline__ void line_bitonic_merge(uint32_t (&v)[NP][32])
 // (T = 5 is line_bitonic_merge).  Used on column registers by the tile mergesort: a block of 2^T
 // rows of the page is a bitonic sequence of 32 * 2^T elements, and its stages of stride >= 32
 // elements are exactly these register stages of the thread that owns the column.
-template <int NP, int T>
+template <int NP, int T, int FMOD = BCF_CE1_FMA_MOD>
 __device__ __forceinline__ void block_bitonic_merge(uint32_t (&v)[NP][32])
 {
 #pragma unroll
     for (int s = (1 << (T - 1)); s >= 1; s >>= 1) {
 #pragma unroll
         for (int k = 0; k < 32; ++k)
-            if ((k & s) == 0) ce<NP>(v, k, k + s);
+            if ((k & s) == 0) ce<NP, FMOD>(v, k, k + s);
     }
 }
 

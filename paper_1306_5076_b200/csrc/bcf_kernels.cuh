@@ -282,6 +282,9 @@ tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vou
 // instead of 2101, the same 10 sweeps through shared memory; the sorted tile is unique, so the
 // result is bit-identical to ShearSort's.  bcf_sort_tiles stays ShearSort (row a2); this kernel is
 // bcf_sort_tiles_mergesort and, by default, the base case of bcf_sort.
+#ifndef BCF_TMS_FMA_MOD
+#define BCF_TMS_FMA_MOD 0     // min/max only: this kernel is not bound by the ALU pipe (A/B in DESIGN.md 5.6)
+#endif
 template <class E, int T>
 __device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lane, uint32_t (&v)[E::NP][32])
 {
@@ -290,18 +293,28 @@ __device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lan
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_load_level<T>(planes + p * TILE, v[p], lane);
-    block_bitonic_merge<E::NP, T>(v);                    // column pass: strides 2^(T-1) .. 1 rows
+    block_bitonic_merge<E::NP, T, BCF_TMS_FMA_MOD>(v);   // column pass: strides 2^(T-1) .. 1 rows
     __syncwarp();                                        // mirrored reads: another thread's words are overwritten next
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
-    line_bitonic_merge<E::NP>(v);                        // row pass: strides 16 .. 1
+    line_bitonic_merge<E::NP, BCF_TMS_FMA_MOD>(v);       // row pass: strides 16 .. 1
 }
 
+// resident CTAs per SM asked of the compiler (register cap), per number of planes
+#ifndef BCF_TMS_MINB1
+#define BCF_TMS_MINB1 4
+#endif
+#ifndef BCF_TMS_MINB2
+#define BCF_TMS_MINB2 4
+#endif
+#ifndef BCF_TMS_MINB3
+#define BCF_TMS_MINB3 3
+#endif
 template <class E>
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32)
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, E::NP == 1 ? BCF_TMS_MINB1 : E::NP == 2 ? BCF_TMS_MINB2 : BCF_TMS_MINB3)
 tile_mergesort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
 {
     extern __shared__ __align__(16) uint32_t smem[];
@@ -317,7 +330,7 @@ tile_mergesort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
         uint32_t v[E::NP][32];
         if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
         else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);
-        line_sort<E::NP>(v);                                // every row ascending
+        line_sort<E::NP, BCF_TMS_FMA_MOD>(v);               // every row ascending
         tile_merge_level<E, 1>(planes, lane, v);
         tile_merge_level<E, 2>(planes, lane, v);
         tile_merge_level<E, 3>(planes, lane, v);
