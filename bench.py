@@ -329,7 +329,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4a", choices=sorted(WORKLOADS))
     ap.add_argument("--log2n", type=int, default=0, help="override the element count (debugging only)")
-    ap.add_argument("--base-case", default="tilemergesort", choices=["shearsort", "tilemergesort"],
+    ap.add_argument("--base-case", default="tilemergesort", choices=["shearsort", "tilemergesort", "longtiles"],
                     help="base case of bcf_sort: the paper's tile ShearSort or the tile mergesort network (default)")
     ap.add_argument("--rounds-per-pass", type=int, default=1, choices=[1, 2],
                     help="merge rounds per pass over global memory (2 = four-run kernel)")
@@ -365,7 +365,8 @@ def main():
 
     global TILE_ALGO
     TILE_ALGO = args.tile_algo
-    bcf.set_base_case(bcf.BASE_SHEARSORT if args.base_case == "shearsort" else bcf.BASE_TILE_MERGESORT)
+    bcf.set_base_case({"shearsort": bcf.BASE_SHEARSORT, "tilemergesort": bcf.BASE_TILE_MERGESORT,
+                       "longtiles": bcf.BASE_LONG_TILES}[args.base_case])
     bcf.set_rounds_per_pass(args.rounds_per_pass)
 
     desc, logn, gen, op, dtype = WORKLOADS[args.workload]

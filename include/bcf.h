@@ -109,12 +109,25 @@ bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles
                                     bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
 
 /*
+ * bcf_sort_long_tiles -- long tiles M = h * w^2 (section 3.1, Appendix E): every
+ * group of h consecutive tiles (h = 2, 4 or 8; h divides w) is sorted as ONE sequence of 1024 h
+ * elements by the h warps of one CTA without leaving the chip: each warp sorts its tile, then
+ * log2 h rounds merge the sorted tiles pairwise with the data-oblivious form of the paper's page
+ * merge (flip stage + half-cleaners between tiles through conflict-free shared memory, then the
+ * column pass and row pass inside each tile).  The paper's own nested Segmented ShearSort
+ * (Alg. 3-5) is not used.  In place; long tile t = elements [1024 h t, 1024 h (t+1)).
+ */
+bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles, int h,
+                               bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
+
+/*
  * Base case bcf_sort uses from now on (process-wide, host only): BCF_BASE_SHEARSORT = the paper's
- * tile ShearSort (bcf_sort_tiles), BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort.  The result
+ * tile ShearSort (bcf_sort_tiles), BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort,
+ * BCF_BASE_LONG_TILES = bcf_sort_long_tiles with h = 8 (runs of 8192, three merge rounds fewer).  The result
  * of bcf_sort is the same for both.  Initial value: BCF_BASE_TILE_MERGESORT, or the integer in the
  * environment variable BCF_BASE_CASE.
  */
-typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1 } bcf_base_case;
+typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2 } bcf_base_case;
 bcf_status bcf_set_base_case(int base);
 int bcf_get_base_case(void);
 

@@ -36,6 +36,8 @@ from .binding import (  # noqa: F401
     get_base_case,
     BASE_SHEARSORT,
     BASE_TILE_MERGESORT,
+    BASE_LONG_TILES,
+    sort_long_tiles,
     version,
     workspace_bytes,
 )

@@ -42,6 +42,7 @@ def lib():
     L.bcf_sort_tiles.argtypes = [vp, vp, sz, ci, ci, vp]
     L.bcf_sort_tiles_mergesort.argtypes = [vp, vp, sz, ci, ci, vp]
     L.bcf_set_base_case.argtypes = [ci]
+    L.bcf_sort_long_tiles.argtypes = [vp, vp, sz, ci, ci, ci, vp]
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
@@ -153,7 +154,18 @@ def sort_tiles_mergesort(keys, vals=None, stream=None):
     return keys if vals is None else (keys, vals)
 
 
-BASE_SHEARSORT, BASE_TILE_MERGESORT = 0, 1
+def sort_long_tiles(keys, h, vals=None, stream=None):
+    """bcf_sort_long_tiles: in place sort of consecutive long tiles of 1024 * h elements (h = 2, 4, 8)."""
+    kt, vt = _types(keys, vals)
+    n = keys.numel()
+    if h not in (2, 4, 8) or n % (TILE * h):
+        raise ValueError("sort_long_tiles needs h in (2, 4, 8) and a whole number of 1024*h-element long tiles")
+    _check(lib().bcf_sort_long_tiles(_dev(keys, "keys"), _dev(vals, "vals"), n // (TILE * h), int(h), kt, vt,
+                                     _stream(stream)), "bcf_sort_long_tiles")
+    return keys if vals is None else (keys, vals)
+
+
+BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES = 0, 1, 2
 
 
 def set_base_case(base):

@@ -10,6 +10,7 @@
 #include "bcf_pagewise.cuh"
 #include "bcf_merge_pipe.cuh"
 #include "bcf_merge4.cuh"
+#include "bcf_long_tile.cuh"
 #include <cstdlib>
 
 using namespace bcf;
@@ -121,8 +122,8 @@ inline int base_case()
 {
     if (g_base_case < 0) {
         const char *e = std::getenv("BCF_BASE_CASE");
-        g_base_case = e ? (std::atoi(e) == BCF_BASE_SHEARSORT ? BCF_BASE_SHEARSORT : BCF_BASE_TILE_MERGESORT)
-                        : BCF_DEFAULT_BASE_CASE;
+        const int v = e ? std::atoi(e) : BCF_DEFAULT_BASE_CASE;
+        g_base_case = (v >= BCF_BASE_SHEARSORT && v <= BCF_BASE_LONG_TILES) ? v : BCF_DEFAULT_BASE_CASE;
     }
     return g_base_case;
 }
@@ -150,6 +151,48 @@ bcf_status launch_tile_sort(const void *kin, const uint32_t *vin, void *kout, ui
             tile_sort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
     }
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+// Long tiles (bcf_long_tile.cuh): groups of h = 2, 4 or 8 tiles sorted by one CTA of h warps.
+#ifndef BCF_LONG_TILE_H
+#define BCF_LONG_TILE_H 8
+#endif
+template <class E, int H>
+bcf_status launch_long_tile_h(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, cudaStream_t s)
+{
+    using C = LongTileCfg<E, H>;
+    static int num_sms = 0, ctas = 0;
+    if (!num_sms) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+            return BCF_ERR_CUDA;
+        if (cudaFuncSetAttribute(long_tile_sort_kernel<E, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, long_tile_sort_kernel<E, H>, H * 32, C::smem) != cudaSuccess ||
+            ctas < 1) {
+            num_sms = 0;
+            return BCF_ERR_CUDA;
+        }
+    }
+    const size_t groups = ((n + TILE - 1) / TILE + H - 1) / H;
+    if (groups == 0) return BCF_OK;
+    const size_t cap = static_cast<size_t>(ctas) * num_sms * 8;     // a few waves; the kernel strides over groups
+    {
+        LaunchTimer t(BCF_KERNEL_TILE_SORT, s);
+        long_tile_sort_kernel<E, H><<<static_cast<unsigned>(groups < cap ? groups : cap), H * 32, C::smem, s>>>(kin, vin, kout, vout, n);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+template <class E>
+bcf_status launch_long_tile(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, int h, cudaStream_t s)
+{
+    switch (h) {
+    case 2: return launch_long_tile_h<E, 2>(kin, vin, kout, vout, n, s);
+    case 4: return launch_long_tile_h<E, 4>(kin, vin, kout, vout, n, s);
+    case 8: return launch_long_tile_h<E, 8>(kin, vin, kout, vout, n, s);
+    }
+    return BCF_ERR_INVALID_ARG;
 }
 
 template <class E>
@@ -578,9 +621,24 @@ bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles
     return sort_tiles_common(d_keys, d_vals, num_tiles, kt, vt, stream, BCF_BASE_TILE_MERGESORT);
 }
 
+bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles, int h, bcf_key_t kt, bcf_val_t vt,
+                               bcf_stream_t stream)
+{
+    if (!valid_types(kt, vt) || (h != 2 && h != 4 && h != 8)) return BCF_ERR_INVALID_ARG;
+    if (num_long_tiles == 0) return BCF_OK;
+    if (num_long_tiles * h >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys) || !aligned16(d_vals)) return BCF_ERR_MISALIGNED;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(d_keys, static_cast<uint32_t *>(d_vals), d_keys, static_cast<uint32_t *>(d_vals),
+                                                  num_long_tiles * h * TILE, h, stream));
+    return st;
+}
+
 bcf_status bcf_set_base_case(int base)
 {
-    if (base != BCF_BASE_SHEARSORT && base != BCF_BASE_TILE_MERGESORT) return BCF_ERR_INVALID_ARG;
+    if (base < BCF_BASE_SHEARSORT || base > BCF_BASE_LONG_TILES) return BCF_ERR_INVALID_ARG;
     g_base_case = base;
     return BCF_OK;
 }
@@ -665,19 +723,24 @@ bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_
     bcf_status st = check_device();
     if (st != BCF_OK) return st;
 
-    const size_t tiles = (n + TILE - 1) / TILE;
-    const int rounds = ceil_log2(tiles);
-    const Workspace w = carve(d_workspace, n, kt, vt, rounds > 0, rounds > 0 ? max_shares(n, TILE) : 0);
+    // base case: runs of base_run sorted elements (one tile, or a long tile of h tiles)
+    const int bc = base_case();
+    const size_t base_run = (bc == BCF_BASE_LONG_TILES) ? size_t(BCF_LONG_TILE_H) * TILE : size_t(TILE);
+    const int passes = n > base_run ? count_passes(n, base_run, kt, vt) : 0;
+    const Workspace w = carve(d_workspace, n, kt, vt, passes > 0, passes > 0 ? max_shares(n, TILE) : 0);
     uint32_t *vals = static_cast<uint32_t *>(d_vals);
     // With an odd number of merge passes the base case writes into the workspace, so that the
     // last pass lands in the caller's buffer without an extra copy.
-    const bool base_to_ws = (count_passes(n, TILE, kt, vt) % 2 == 1);
+    const bool base_to_ws = (passes % 2 == 1);
     void *k0 = base_to_ws ? w.keys : d_keys;
     uint32_t *v0 = base_to_ws ? w.vals : vals;
-    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream, base_case()));
-    if (st != BCF_OK || rounds == 0) return st;
-    // round 1 writes to the buffer the base case did not write.
-    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, TILE,
+    if (bc == BCF_BASE_LONG_TILES)
+        BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(d_keys, vals, k0, v0, n, BCF_LONG_TILE_H, stream));
+    else
+        BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream, bc));
+    if (st != BCF_OK || passes == 0) return st;
+    // pass 1 writes to the buffer the base case did not write.
+    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, base_run,
                                               w.splits, stream));
     return st;
 }

@@ -30,7 +30,7 @@ def rpp(request, bcf):
     bcf.set_rounds_per_pass(before)
 
 
-@pytest.fixture(params=[0, 1], ids=["shearsort", "tilemergesort"])
+@pytest.fixture(params=[0, 1, 2], ids=["shearsort", "tilemergesort", "longtiles"])
 def base(request, bcf):
     """Both base cases of bcf_sort: the paper's tile ShearSort and the tile mergesort network."""
     before = bcf.get_base_case()
@@ -131,6 +131,26 @@ def test_sort_tiles_mergesort_configs_1_and_2(bcf):
     bcf.sort_tiles_mergesort(dk, dv)
     wk, wv = oracle.shearsort_tiles(keys, vals)
     assert np.array_equal(host(dk, keys), wk) and np.array_equal(host(dv, vals), wv)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("h", [2, 4, 8])
+@pytest.mark.parametrize("groups", [1, 3, 37])
+def test_sort_long_tiles_matches_oracle(bcf, kind, h, groups):
+    """Long tiles h * w^2 (SURVEY 8f item 1): every block of 1024 h elements sorted as one sequence;
+    the oracle sorts each block with its own ShearSort + two-finger merge rounds."""
+    m = 1024 * h
+    keys, vals = make(kind, groups * m, seed=1000 * h + groups, dup=(groups == 3))
+    if groups >= 3:
+        keys[m:2 * m] = keys[m]                                         # all-equal long tile
+        keys[2 * m:3 * m] = np.sort(keys[2 * m:3 * m])[::-1]            # reversed long tile
+    dk, dv = dev(keys), dev(vals)
+    bcf.sort_long_tiles(dk, h, dv)
+    gk, gv = host(dk, keys), None if vals is None else host(dv, vals)
+    for g in range(groups):
+        sl = slice(g * m, (g + 1) * m)
+        want = oracle.sort_full(keys[sl], None if vals is None else vals[sl])
+        assert_same(gk[sl], None if vals is None else gv[sl], want, vals)
 
 
 def test_sort_tiles_config2_shape(bcf):
