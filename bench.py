@@ -5,19 +5,24 @@
 
 A "step" is one pass of the whole hot path over one batch of synthetic input: bcf_sort of
 BASELINE.json config 4 (2^28 uint32 keys, uniform; the configuration the metric's target is quoted
-on) -- base-case ShearSort of 2^18 tiles + 18 merge rounds (partition + merge launch each).
+on) -- base case (default: long tiles of 8192 keys, one CTA of 8 warps each: tile mergesort + 3 on-chip
+merge rounds; --base-case shearsort gives the paper's tile ShearSort) + the remaining merge rounds
+(partition + merge launch each, one round per pass over HBM unless --rounds-per-pass 2).
 Rank 0 prints ONE JSON line (contract in the task statement):
   value     keys/s, device-timed (CUDA events around each bcf_sort call on the launching stream; the
             input is restored from a pristine device copy before each step, outside the events),
             summed over ranks, max-over-ranks time
   e2e       same metric through bcf_sort_host with pinned HOST buffers, H2D + sort + D2H timed
-  roofline  the merge kernel (18 of the 37 launches of a step): algorithmic bytes 2*4*n per launch
+  roofline  the merge kernel (15 of the 31 launches of a step): algorithmic bytes 2*4*n per launch
             over its mean launch duration (CUDA events recorded inside libbcf on the same stream)
             against the measured HBM copy bandwidth of MEASURED_PEAKS.json
   cpu_baseline  the CPU oracle (oracle/, single thread) timed on a bounded sample of the workload
 Multi-GPU: the sort does not shard without an exchange step the paper does not have; --gpus N runs N
 independent replicas ("replicas only"), one process per GPU under torchrun.
 `--impl reference` times the oracle alone (this tier's reference arm).
+`other_workloads` holds short device-timed lines for the other BASELINE.json configs and for the same
+configs with the other networks / pass structures (paper's ShearSort base case, tile mergesort, two merge
+rounds per pass), so the headline never hides what the paper's own base case costs.
 """
 import argparse
 import json
@@ -294,8 +299,27 @@ def time_steps(torch, job, steps, stream, barrier):
     return [a.elapsed_time(b) for a, b in ev]
 
 
-def side_line(bcf, torch, dev, name, stream, barrier):
-    """A short device-timed measurement of another BASELINE.json config (3 warm-ups, 5 steps)."""
+def side_line(bcf, torch, dev, name, stream, barrier, variant=None):
+    """A short device-timed measurement of another BASELINE.json config (3 warm-ups, 5 steps).
+    variant: None, or a dict of library / bench settings for this line only
+    ({"base_case": .., "rounds_per_pass": .., "tile_algo": ..})."""
+    global TILE_ALGO
+    saved = (bcf.get_base_case(), bcf.get_rounds_per_pass(), TILE_ALGO)
+    if variant:
+        if "base_case" in variant:
+            bcf.set_base_case(variant["base_case"])
+        if "rounds_per_pass" in variant:
+            bcf.set_rounds_per_pass(variant["rounds_per_pass"])
+        TILE_ALGO = variant.get("tile_algo", TILE_ALGO)
+    try:
+        return _side_line(bcf, torch, dev, name, stream, barrier, variant)
+    finally:
+        bcf.set_base_case(saved[0])
+        bcf.set_rounds_per_pass(saved[1])
+        TILE_ALGO = saved[2]
+
+
+def _side_line(bcf, torch, dev, name, stream, barrier, variant):
     desc, logn, gen, op, dtype = WORKLOADS[name]
     n = 1 << logn
     job = Job(bcf, torch, dev, name, n)
@@ -316,6 +340,8 @@ def side_line(bcf, torch, dev, name, stream, barrier):
             "ms_per_step": t, "best_ms": min(ms), "passes": passes,
             "frac_of_measured_hbm_peak_for_pass_count": bytes_moved / (t * 1e-3) / 1e9 / peak,
             "gpu_launches_per_step": int(sum(launches.values())) // 5}
+    if variant:
+        line["variant"] = variant.get("label", "")
     del job
     torch.cuda.empty_cache()
     return line
@@ -329,8 +355,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4a", choices=sorted(WORKLOADS))
     ap.add_argument("--log2n", type=int, default=0, help="override the element count (debugging only)")
-    ap.add_argument("--base-case", default="tilemergesort", choices=["shearsort", "tilemergesort", "longtiles"],
-                    help="base case of bcf_sort: the paper's tile ShearSort or the tile mergesort network (default)")
+    ap.add_argument("--base-case", default="auto", choices=["auto", "shearsort", "tilemergesort", "longtiles"],
+                    help="base case of bcf_sort: the paper's tile ShearSort, the tile mergesort network, long tiles "
+                         "(8 tiles per CTA), or auto = the library default (long tiles for u32 keys, tile mergesort else)")
     ap.add_argument("--rounds-per-pass", type=int, default=1, choices=[1, 2],
                     help="merge rounds per pass over global memory (2 = four-run kernel)")
     ap.add_argument("--tile-algo", default="shearsort", choices=["shearsort", "mergesort"],
@@ -366,7 +393,7 @@ def main():
     global TILE_ALGO
     TILE_ALGO = args.tile_algo
     bcf.set_base_case({"shearsort": bcf.BASE_SHEARSORT, "tilemergesort": bcf.BASE_TILE_MERGESORT,
-                       "longtiles": bcf.BASE_LONG_TILES}[args.base_case])
+                       "longtiles": bcf.BASE_LONG_TILES, "auto": bcf.BASE_AUTO}[args.base_case])
     bcf.set_rounds_per_pass(args.rounds_per_pass)
 
     desc, logn, gen, op, dtype = WORKLOADS[args.workload]
@@ -484,6 +511,17 @@ def main():
         del job
         torch.cuda.empty_cache()
         side = [side_line(bcf, torch, dev, w, stream, barrier) for w in SIDE_WORKLOADS]
+        # the same configs with the other networks / pass structures the library offers
+        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
+                              {"base_case": bcf.BASE_SHEARSORT, "label": "base case = the paper's tile ShearSort"}))
+        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
+                              {"base_case": bcf.BASE_TILE_MERGESORT, "label": "base case = tile mergesort (one tile per warp)"}))
+        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
+                              {"rounds_per_pass": 2, "label": "two merge rounds per pass (four-run kernel)"}))
+        side.append(side_line(bcf, torch, dev, "cfg1", stream, barrier,
+                              {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
+        side.append(side_line(bcf, torch, dev, "cfg2", stream, barrier,
+                              {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
 
     if rank == 0:
         print(json.dumps({
@@ -491,7 +529,9 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
             "config": {"workload": args.workload, "description": desc, "n": n, "bytes": eb * n,
-                       "passes": passes, "base_case": args.base_case if op == "sort" else None,
+                       "passes": passes,
+                       "base_case": None if op != "sort" else (args.base_case if args.base_case != "auto" else
+                                                               "auto: " + ("longtiles" if dtype == "u32" else "tilemergesort")),
                        "tile_network": args.tile_algo if op == "tiles" else None,
                        "merge_rounds_per_pass": args.rounds_per_pass, "multi_gpu": "replicas only",
                        "l2": "input and workspace (%d MiB each) %s the 126 MB L2; the input is restored from a "

@@ -123,11 +123,13 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
 /*
  * Base case bcf_sort uses from now on (process-wide, host only): BCF_BASE_SHEARSORT = the paper's
  * tile ShearSort (bcf_sort_tiles), BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort,
- * BCF_BASE_LONG_TILES = bcf_sort_long_tiles with h = 8 (runs of 8192, three merge rounds fewer).  The result
- * of bcf_sort is the same for both.  Initial value: BCF_BASE_TILE_MERGESORT, or the integer in the
+ * BCF_BASE_LONG_TILES = bcf_sort_long_tiles with h = 8 (runs of 8192, three merge rounds fewer),
+ * BCF_BASE_AUTO = the fastest measured on B200 per element type (long tiles for u32 keys alone, the tile
+ * mergesort otherwise).  The result
+ * of bcf_sort is the same for both.  Initial value: BCF_BASE_AUTO, or the integer in the
  * environment variable BCF_BASE_CASE.
  */
-typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2 } bcf_base_case;
+typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2, BCF_BASE_AUTO = 3 } bcf_base_case;
 bcf_status bcf_set_base_case(int base);
 int bcf_get_base_case(void);
 

@@ -37,6 +37,7 @@ from .binding import (  # noqa: F401
     BASE_SHEARSORT,
     BASE_TILE_MERGESORT,
     BASE_LONG_TILES,
+    BASE_AUTO,
     sort_long_tiles,
     version,
     workspace_bytes,

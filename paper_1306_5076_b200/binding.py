@@ -165,7 +165,7 @@ def sort_long_tiles(keys, h, vals=None, stream=None):
     return keys if vals is None else (keys, vals)
 
 
-BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES = 0, 1, 2
+BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES, BASE_AUTO = 0, 1, 2, 3
 
 
 def set_base_case(base):

@@ -112,10 +112,11 @@ struct LaunchTimer {
 template <class E>
 constexpr size_t warp_smem_bytes() { return size_t(E::NP) * TILE * 4; }
 
-// Base case of bcf_sort: BCF_BASE_SHEARSORT (the paper's tile sort) or BCF_BASE_TILE_MERGESORT (same
-// tile, same movement, mergers instead of full line sorts; bcf_kernels.cuh).  bcf_set_base_case().
+// Base case of bcf_sort: BCF_BASE_SHEARSORT (the paper's tile sort), BCF_BASE_TILE_MERGESORT (same tile,
+// same movement, mergers instead of full line sorts; bcf_kernels.cuh), BCF_BASE_LONG_TILES (8 tiles per CTA,
+// bcf_long_tile.cuh) or BCF_BASE_AUTO.  bcf_set_base_case().
 #ifndef BCF_DEFAULT_BASE_CASE
-#define BCF_DEFAULT_BASE_CASE BCF_BASE_TILE_MERGESORT
+#define BCF_DEFAULT_BASE_CASE BCF_BASE_AUTO
 #endif
 int g_base_case = -1;
 inline int base_case()
@@ -123,7 +124,7 @@ inline int base_case()
     if (g_base_case < 0) {
         const char *e = std::getenv("BCF_BASE_CASE");
         const int v = e ? std::atoi(e) : BCF_DEFAULT_BASE_CASE;
-        g_base_case = (v >= BCF_BASE_SHEARSORT && v <= BCF_BASE_LONG_TILES) ? v : BCF_DEFAULT_BASE_CASE;
+        g_base_case = (v >= BCF_BASE_SHEARSORT && v <= BCF_BASE_AUTO) ? v : BCF_DEFAULT_BASE_CASE;
     }
     return g_base_case;
 }
@@ -638,7 +639,7 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
 
 bcf_status bcf_set_base_case(int base)
 {
-    if (base < BCF_BASE_SHEARSORT || base > BCF_BASE_LONG_TILES) return BCF_ERR_INVALID_ARG;
+    if (base < BCF_BASE_SHEARSORT || base > BCF_BASE_AUTO) return BCF_ERR_INVALID_ARG;
     g_base_case = base;
     return BCF_OK;
 }
@@ -724,7 +725,9 @@ bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_
     if (st != BCF_OK) return st;
 
     // base case: runs of base_run sorted elements (one tile, or a long tile of h tiles)
-    const int bc = base_case();
+    // AUTO: what measures fastest on B200 -- long tiles for 4-byte keys alone, the tile mergesort otherwise
+    int bc = base_case();
+    if (bc == BCF_BASE_AUTO) bc = (kt == BCF_KEY_U32 && vt == BCF_VAL_NONE) ? BCF_BASE_LONG_TILES : BCF_BASE_TILE_MERGESORT;
     const size_t base_run = (bc == BCF_BASE_LONG_TILES) ? size_t(BCF_LONG_TILE_H) * TILE : size_t(TILE);
     const int passes = n > base_run ? count_passes(n, base_run, kt, vt) : 0;
     const Workspace w = carve(d_workspace, n, kt, vt, passes > 0, passes > 0 ? max_shares(n, TILE) : 0);

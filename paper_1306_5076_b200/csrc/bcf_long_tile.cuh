@@ -17,11 +17,15 @@
 //       position p;
 //     * now every tile holds a bitonic sequence and the tiles are in order: column pass and row pass
 //       of SHEARSORT-MERGE inside each tile (2 x 80 comparators per thread).
-//   A cross-tile stage costs one min OR max per element: the warp writes its rows to its own planes
-//   (8 STS.128), a CTA barrier, reads the partner's rows (8 LDS.128, row 31-r and registers reversed
+//   A cross-tile stage costs one min OR max per element: the warp writes its rows to an exchange set
+//   (8 STS.128), one CTA barrier, reads the partner's rows (8 LDS.128, row 31-r and registers reversed
 //   for the flip) -- all conflict-free by the same layout argument as row_store / row_load.
 #pragma once
 #include "bcf_kernels.cuh"
+
+#ifndef BCF_LT_MINB8
+#define BCF_LT_MINB8 2
+#endif
 
 namespace bcf {
 
@@ -62,18 +66,20 @@ __device__ __forceinline__ void cross_stage_keep(const uint32_t *partner, const 
     }
 }
 
+// Two sets of planes used alternately: the barrier of stage s + 1 also tells that every read of
+// stage s is over, so the set written in stage s can be overwritten in stage s + 2 -- one CTA
+// barrier per stage.
 template <class E, bool FLIP>
-__device__ __forceinline__ void cross_stage(uint32_t *smem, const int warp, const int partner, const bool low, const int lane,
+__device__ __forceinline__ void cross_stage(uint32_t *set, const int warp, const int partner, const bool low, const int lane,
                                             uint32_t (&v)[E::NP][32])
 {
-    uint32_t *mine = smem + warp * (E::NP * TILE);
+    uint32_t *mine = set + warp * (E::NP * TILE);
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) row_store(mine + p * TILE, v[p], lane);
     __syncthreads();
-    const uint32_t *other = smem + partner * (E::NP * TILE);
+    const uint32_t *other = set + partner * (E::NP * TILE);
     if (low) cross_stage_keep<E, FLIP, true>(other, lane, v);
     else cross_stage_keep<E, FLIP, false>(other, lane, v);
-    __syncthreads();      // every read of the planes is done before anyone overwrites them
 }
 
 // column pass + row pass on a tile that holds a bitonic sequence in row registers
@@ -96,9 +102,10 @@ __device__ __forceinline__ void tile_bitonic_merge(uint32_t *planes, const int l
 
 template <class E, int H>
 struct LongTileCfg {
-    static constexpr size_t smem = size_t(H) * E::NP * TILE * 4;
+    static constexpr size_t set_words = size_t(H) * E::NP * TILE;
+    static constexpr size_t smem = 2 * set_words * 4;      // two exchange sets
     // resident CTAs the register cap is chosen for
-    static constexpr int min_ctas = (E::NP == 1) ? (H >= 8 ? 2 : 4) : (E::NP == 2 ? (H >= 8 ? 1 : 2) : 1);
+    static constexpr int min_ctas = (E::NP == 1) ? (H >= 8 ? BCF_LT_MINB8 : 4) : (E::NP == 2 ? (H >= 8 ? 1 : 2) : 1);
 };
 
 template <class E, int H>
@@ -108,7 +115,10 @@ long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
     extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    uint32_t *planes = smem + warp * (E::NP * TILE);
+    constexpr size_t SET = LongTileCfg<E, H>::set_words;
+    // A warp's working planes (transposes inside its tile) are its own slot of the set the NEXT stage
+    // writes: its last readers passed a barrier since.
+    uint32_t *const slot = smem + warp * (E::NP * TILE);
     const size_t num_tiles = (n + TILE - 1) / TILE;
     const size_t num_groups = (num_tiles + H - 1) / H;
 
@@ -119,21 +129,23 @@ long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
         if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
         else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);    // missing elements: the maximum element
         line_sort<E::NP, BCF_TMS_FMA_MOD>(v);
-        tile_merge_level<E, 1>(planes, lane, v);
-        tile_merge_level<E, 2>(planes, lane, v);
-        tile_merge_level<E, 3>(planes, lane, v);
-        tile_merge_level<E, 4>(planes, lane, v);
-        tile_merge_level<E, 5>(planes, lane, v);
+        tile_merge_level<E, 1>(slot, lane, v);
+        tile_merge_level<E, 2>(slot, lane, v);
+        tile_merge_level<E, 3>(slot, lane, v);
+        tile_merge_level<E, 4>(slot, lane, v);
+        tile_merge_level<E, 5>(slot, lane, v);
+        int stage = 0;
 #pragma unroll
         for (int B = 2; B <= H; B *= 2) {
             const int i = warp & (B - 1);
-            cross_stage<E, true>(smem, warp, (warp - i) + (B - 1 - i), i < B / 2, lane, v);
+            cross_stage<E, true>(smem + (stage++ & 1) * SET, warp, (warp - i) + (B - 1 - i), i < B / 2, lane, v);
 #pragma unroll
-            for (int s = B / 4; s >= 1; s /= 2) cross_stage<E, false>(smem, warp, warp ^ s, (warp & s) == 0, lane, v);
-            tile_bitonic_merge<E>(planes, lane, v);
+            for (int s = B / 4; s >= 1; s /= 2)
+                cross_stage<E, false>(smem + (stage++ & 1) * SET, warp, warp ^ s, (warp & s) == 0, lane, v);
+            tile_bitonic_merge<E>(slot + (stage & 1) * SET, lane, v);
         }
-        if (cnt > 0) store_rows<E>(planes, kout, vout, base, cnt, cnt == TILE, lane, v);
-        __syncthreads();     // the planes are reused by the CTA's next group
+        if (cnt > 0) store_rows<E>(slot + (stage & 1) * SET, kout, vout, base, cnt, cnt == TILE, lane, v);
+        __syncthreads();     // the exchange sets are reused by the CTA's next group
     }
 }
 
