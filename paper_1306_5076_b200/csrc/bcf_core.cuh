@@ -91,7 +91,8 @@ __device__ __forceinline__ void ce(uint32_t (&v)[NP][32], const int i, const int
         const uint32_t a = v[0][i], b = v[0][j];
         const uint32_t lo = min(a, b);
         v[0][i] = lo;
-        const bool fma = FMOD > 0 && (i % (FMOD > 0 ? FMOD : 1)) != 0;
+        // FMOD > 0: comparators with i % FMOD != 0; FMOD < 0: comparators with i % -FMOD == 0 (a smaller share)
+        const bool fma = FMOD > 0 ? (i % (FMOD > 0 ? FMOD : 1)) != 0 : (FMOD < 0 && (i % (FMOD < 0 ? -FMOD : 1)) == 0);
         v[0][j] = fma ? other_of(a, b, lo) : max(a, b);
     } else {
         const bool sw = elem_gt<NP>(v, i, j);

@@ -285,7 +285,7 @@ tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vou
 #ifndef BCF_TMS_FMA_MOD
 #define BCF_TMS_FMA_MOD 0     // min/max only: this kernel is not bound by the ALU pipe (A/B in DESIGN.md 5.6)
 #endif
-template <class E, int T>
+template <class E, int T, int FM = BCF_TMS_FMA_MOD>
 __device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lane, uint32_t (&v)[E::NP][32])
 {
 #pragma unroll
@@ -293,14 +293,14 @@ __device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lan
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_load_level<T>(planes + p * TILE, v[p], lane);
-    block_bitonic_merge<E::NP, T, BCF_TMS_FMA_MOD>(v);   // column pass: strides 2^(T-1) .. 1 rows
+    block_bitonic_merge<E::NP, T, FM>(v);                // column pass: strides 2^(T-1) .. 1 rows
     __syncwarp();                                        // mirrored reads: another thread's words are overwritten next
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
-    line_bitonic_merge<E::NP, BCF_TMS_FMA_MOD>(v);       // row pass: strides 16 .. 1
+    line_bitonic_merge<E::NP, FM>(v);                    // row pass: strides 16 .. 1
 }
 
 // resident CTAs per SM asked of the compiler (register cap), per number of planes

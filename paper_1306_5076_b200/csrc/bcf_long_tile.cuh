@@ -26,6 +26,11 @@
 #ifndef BCF_LT_MINB8
 #define BCF_LT_MINB8 2
 #endif
+// share of the max outputs formed on the FMA pipe (bcf_core.cuh ce<>): with 8 warps in lock step per
+// CTA this kernel is bound by the ALU pipe, so the offload pays here (A/B in DESIGN.md 5.7)
+#ifndef BCF_LT_FMA_MOD
+#define BCF_LT_FMA_MOD 2
+#endif
 
 namespace bcf {
 
@@ -91,13 +96,13 @@ __device__ __forceinline__ void tile_bitonic_merge(uint32_t *planes, const int l
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_load<false>(planes + p * TILE, v[p], lane);
-    line_bitonic_merge<E::NP, BCF_TMS_FMA_MOD>(v);
+    line_bitonic_merge<E::NP, BCF_LT_FMA_MOD>(v);
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
     __syncwarp();
 #pragma unroll
     for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
-    line_bitonic_merge<E::NP, BCF_TMS_FMA_MOD>(v);
+    line_bitonic_merge<E::NP, BCF_LT_FMA_MOD>(v);
 }
 
 template <class E, int H>
@@ -128,12 +133,12 @@ long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
         uint32_t v[E::NP][32];
         if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
         else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);    // missing elements: the maximum element
-        line_sort<E::NP, BCF_TMS_FMA_MOD>(v);
-        tile_merge_level<E, 1>(slot, lane, v);
-        tile_merge_level<E, 2>(slot, lane, v);
-        tile_merge_level<E, 3>(slot, lane, v);
-        tile_merge_level<E, 4>(slot, lane, v);
-        tile_merge_level<E, 5>(slot, lane, v);
+        line_sort<E::NP, BCF_LT_FMA_MOD>(v);
+        tile_merge_level<E, 1, BCF_LT_FMA_MOD>(slot, lane, v);
+        tile_merge_level<E, 2, BCF_LT_FMA_MOD>(slot, lane, v);
+        tile_merge_level<E, 3, BCF_LT_FMA_MOD>(slot, lane, v);
+        tile_merge_level<E, 4, BCF_LT_FMA_MOD>(slot, lane, v);
+        tile_merge_level<E, 5, BCF_LT_FMA_MOD>(slot, lane, v);
         int stage = 0;
 #pragma unroll
         for (int B = 2; B <= H; B *= 2) {
