@@ -252,8 +252,10 @@ typedef enum {
 
 /*
  * Per-kernel timing with CUDA events recorded on the launching stream (bench.py's `roofline`).
- * bcf_profile_enable(1) makes every later launch be bracketed by an event pair owned by the
- * library (a fixed pool; when it is exhausted further launches are not timed);
+ * bcf_profile_enable(1) makes the library record one event of its own before every later launch
+ * and one at the end of the API call; a launch is timed from its event to the next one, so its
+ * figure includes the gap to the following launch (a fixed pool; when it is exhausted further
+ * launches are not timed);
  * bcf_profile_read synchronises those events, adds up elapsed milliseconds and launch counts
  * per kernel class into ms[BCF_KERNEL_CLASSES] / launches[BCF_KERNEL_CLASSES] (host arrays), and
  * resets the pool.  bcf_profile_enable(0) switches timing off.  Launch COUNTS per class are kept

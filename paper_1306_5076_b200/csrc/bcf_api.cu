@@ -74,36 +74,54 @@ bool overlap(const void *a, size_t an, const void *b, size_t bn)
 
 // ------------------------------------------------------------------ profiling (bcf_profile_*)
 
+// One event per launch, recorded just before it; a launch ends where the next one of the same API call
+// begins, and the last one where the call's closing event (ProfileGroup) is recorded.  One event between
+// two kernels instead of two halves what the instrumentation costs the timed region.
 constexpr int PROFILE_POOL = 8192;
 struct Profile {
     bool on = false;
     int used = 0;
-    cudaEvent_t start[PROFILE_POOL];
-    cudaEvent_t stop[PROFILE_POOL];
-    int cls[PROFILE_POOL];
+    cudaEvent_t ev[PROFILE_POOL];
+    int cls[PROFILE_POOL];             // kernel class of the launch that starts at ev[i]; -1: closing event
     int created = 0;
+    int open_since = -1;               // first entry of the API call in progress
     unsigned long long launches[BCF_KERNEL_CLASSES] = {0, 0, 0, 0};
 } g_prof;
 
+inline int profile_mark(int cls, cudaStream_t s)
+{
+    if (!g_prof.on || g_prof.used >= PROFILE_POOL) return -1;
+    const int idx = g_prof.used++;
+    if (idx >= g_prof.created) {
+        cudaEventCreate(&g_prof.ev[idx]);
+        g_prof.created = idx + 1;
+    }
+    g_prof.cls[idx] = cls;
+    cudaEventRecord(g_prof.ev[idx], s);
+    return idx;
+}
+
 struct LaunchTimer {
-    int idx = -1;
-    cudaStream_t s;
-    LaunchTimer(int cls, cudaStream_t stream) : s(stream)
+    LaunchTimer(int cls, cudaStream_t stream)
     {
         g_prof.launches[cls]++;
-        if (!g_prof.on || g_prof.used >= PROFILE_POOL) return;
-        idx = g_prof.used++;
-        if (idx >= g_prof.created) {
-            cudaEventCreate(&g_prof.start[idx]);
-            cudaEventCreate(&g_prof.stop[idx]);
-            g_prof.created = idx + 1;
-        }
-        g_prof.cls[idx] = cls;
-        cudaEventRecord(g_prof.start[idx], s);
+        profile_mark(cls, stream);
     }
-    ~LaunchTimer()
+};
+
+// Closes the timed launches of one public API call (outermost scope only).
+struct ProfileGroup {
+    cudaStream_t s;
+    bool outer;
+    explicit ProfileGroup(cudaStream_t stream) : s(stream), outer(g_prof.open_since < 0)
     {
-        if (idx >= 0) cudaEventRecord(g_prof.stop[idx], s);
+        if (outer) g_prof.open_since = g_prof.used;
+    }
+    ~ProfileGroup()
+    {
+        if (!outer) return;
+        if (g_prof.used > g_prof.open_since && g_prof.cls[g_prof.used - 1] >= 0) profile_mark(-1, s);
+        g_prof.open_since = -1;
     }
 };
 
@@ -502,6 +520,7 @@ bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d
                              void *d_vals_out, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
                              void *d_workspace, size_t workspace_bytes, cudaStream_t s)
 {
+    ProfileGroup profile_group(s);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
@@ -599,6 +618,7 @@ size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_v
 static bcf_status sort_tiles_common(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream,
                                     int algo)
 {
+    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (num_tiles == 0) return BCF_OK;
     if (num_tiles >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
@@ -625,6 +645,7 @@ bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles
 bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles, int h, bcf_key_t kt, bcf_val_t vt,
                                bcf_stream_t stream)
 {
+    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt) || (h != 2 && h != 4 && h != 8)) return BCF_ERR_INVALID_ARG;
     if (num_long_tiles == 0) return BCF_OK;
     if (num_long_tiles * h >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
@@ -649,6 +670,7 @@ int bcf_get_base_case(void) { return base_case(); }
 bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
                                bcf_val_t vt, uint32_t *d_splits, size_t num_shares, bcf_stream_t stream)
 {
+    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
@@ -665,6 +687,7 @@ bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, siz
 bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
                                 bcf_val_t vt, uint32_t *d_splits, size_t num_bounds, bcf_stream_t stream)
 {
+    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
@@ -712,6 +735,7 @@ bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in,
 bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_workspace,
                     size_t workspace_bytes, bcf_stream_t stream)
 {
+    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32)) return BCF_ERR_INVALID_ARG;
@@ -779,6 +803,7 @@ bcf_status bcf_profile_enable(int on)
 {
     g_prof.on = on != 0;
     g_prof.used = 0;
+    g_prof.open_since = -1;
     return BCF_OK;
 }
 
@@ -786,10 +811,11 @@ bcf_status bcf_profile_read(float *ms, unsigned long long *launches)
 {
     if (!ms || !launches) return BCF_ERR_INVALID_ARG;
     for (int c = 0; c < BCF_KERNEL_CLASSES; ++c) { ms[c] = 0.f; launches[c] = 0; }
-    for (int i = 0; i < g_prof.used; ++i) {
-        if (cudaEventSynchronize(g_prof.stop[i]) != cudaSuccess) return BCF_ERR_CUDA;
+    for (int i = 0; i + 1 < g_prof.used; ++i) {
+        if (g_prof.cls[i] < 0) continue;
+        if (cudaEventSynchronize(g_prof.ev[i + 1]) != cudaSuccess) return BCF_ERR_CUDA;
         float t = 0.f;
-        if (cudaEventElapsedTime(&t, g_prof.start[i], g_prof.stop[i]) != cudaSuccess) return BCF_ERR_CUDA;
+        if (cudaEventElapsedTime(&t, g_prof.ev[i], g_prof.ev[i + 1]) != cudaSuccess) return BCF_ERR_CUDA;
         ms[g_prof.cls[i]] += t;
         launches[g_prof.cls[i]]++;
     }
