@@ -169,6 +169,32 @@ bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, si
                                 bcf_stream_t stream);
 
 /*
+ * bcf_find_buckets -- FIND-BUCKETS, the paper's deterministic bucket distribution (section 3.2
+ * "Distribution" L131-137, Lemma 1, Algorithm 7), with the pivot buckets of
+ * section 3.3 (L155, BCFMergesortPB) as an option.  Not on the hot path (bcf_merge_runs partitions
+ * by exact co-ranking); provided as the paper's own partitioner.  Keys only.
+ *   d_keys_in  : n keys, s = ceil(n / run_len) sorted runs of run_len (the last may be shorter).
+ *   t          : samples per run; sample i of run r is its element floor(i * len_r / t).
+ *   P          : buckets.  The s*t samples are sorted; pivot j = sorted sample floor((j+1) s t / P),
+ *                j = 0..P-2.  Bucket j holds the keys with pivot[j-1] < key <= pivot[j].
+ *   pivot_buckets != 0 : keys equal to pivot j get a bucket of their own right after bucket j
+ *                (which then holds pivot[j-1] < key < pivot[j]): nb = 2P-1 buckets instead of nb = P;
+ *                the second copy of a repeated pivot owns nothing.
+ *   d_keys_out : n keys: the runs' pieces regrouped by bucket, inside a bucket by run, every piece
+ *                in its original (sorted) order.  Buckets are in ascending key order.
+ *   d_pivots   : P-1 keys.
+ *   d_piece_offsets : nb*s + 1 uint32: entry b*s + r = position in d_keys_out of the piece of run r
+ *                in bucket b; the last entry is n.  (Bucket b starts at entry b*s.)
+ *   d_workspace: >= bcf_find_buckets_workspace_bytes(...) bytes.
+ * Lemma 1: with all keys distinct every bucket has at most s*ceil(len/t) + ceil(s t / P)*ceil(len/t)
+ * keys, len = run_len.  Requires t >= 1, P >= 2, s*t >= P, s, t, P <= 65536.
+ */
+size_t bcf_find_buckets_workspace_bytes(size_t n, size_t run_len, int t, int P, int pivot_buckets, bcf_key_t kt);
+bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int t, int P, int pivot_buckets,
+                            bcf_key_t kt, void *d_keys_out, void *d_pivots, uint32_t *d_piece_offsets,
+                            void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+
+/*
  * Number of passes over global memory (one read + one write of all n elements each) that
  * bcf_merge_runs takes from runs of run_len: a pass does two merge rounds where the four-run
  * kernel applies (run_len = 1024 * 2^k and the element type's stage buffers fit one SM) and one

@@ -171,3 +171,49 @@ def corank_multi(runs_keys, d, runs_vals=None):
     first = order[:d]
     bounds = np.cumsum([0] + lens)
     return [int(np.count_nonzero((first >= bounds[r]) & (first < bounds[r + 1]))) for r in range(len(ks))]
+
+
+def find_buckets(keys, run_len, t, P, pivot_buckets=False):
+    """FIND-BUCKETS, section 3.2 "Distribution" (L131-137) / Algorithm 7 (L492-520), with the
+    pivot buckets of L155 as an option; reading A18 of DESIGN.md for the garbled lines.  Step by step:
+      1. S: t samples of each of the s sorted runs, sample i of run r = its element floor(i len_r / t)
+         (Alg. 7 L503: "S[pid t + i] = I_pid[i n/t]");
+      2. MERGESORT(S) (L505) -- a library sort serves as the step;
+      3. pivots F[j] = S[floor((j+1) s t / P)], j = 0..P-2 ("P-1 evenly spaced items from S", L135);
+      4. rank of every pivot in every run = number of elements <= pivot (L507-510: first i with
+         I[i] > F[c]); with pivot buckets also the number of elements < pivot;
+      5. bucket sizes summed over the runs, exclusive prefix sums (L512-513);
+      6. O = the runs' pieces regrouped by bucket, inside a bucket by run (L515-520).
+    Keys only.  Returns (O, F, Q) with Q[b s + r] = start of piece (bucket b, run r) in O, Q[-1] = n."""
+    k = np.ascontiguousarray(keys)
+    _suffix(k)
+    n = k.size
+    s = -(-n // run_len)
+    runs = [k[r * run_len:min(n, (r + 1) * run_len)] for r in range(s)]
+    S = np.array([run[(i * run.size) // t] for run in runs for i in range(t)], dtype=k.dtype)
+    S = np.sort(S, kind="stable")
+    F = np.array([S[((j + 1) * s * t) // P] for j in range(P - 1)], dtype=k.dtype)
+    nb = 2 * P - 1 if pivot_buckets else P
+    bounds = np.zeros((s, nb + 1), dtype=np.int64)
+    for r, run in enumerate(runs):
+        le = np.searchsorted(run, F, side="right")
+        if not pivot_buckets:
+            bounds[r, 1:P] = le
+        else:
+            lt = np.searchsorted(run, F, side="left")
+            for j in range(P - 1):
+                dup = j > 0 and F[j] == F[j - 1]        # the second copy of a repeated pivot owns nothing
+                bounds[r, 2 * j + 1] = le[j] if dup else lt[j]
+                bounds[r, 2 * j + 2] = le[j]
+        bounds[r, nb] = run.size
+    O = np.empty_like(k)
+    Q = np.zeros(nb * s + 1, dtype=np.int64)
+    oc = 0
+    for b in range(nb):
+        for r, run in enumerate(runs):
+            piece = run[bounds[r, b]:bounds[r, b + 1]]
+            Q[b * s + r] = oc
+            O[oc:oc + piece.size] = piece
+            oc += piece.size
+    Q[nb * s] = oc
+    return O, F, Q

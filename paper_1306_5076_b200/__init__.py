@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     layout_access,
     layout_word,
     lib,
+    find_buckets,
     merge_partition,
     merge_partition4,
     merge_pass_count,

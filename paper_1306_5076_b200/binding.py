@@ -46,6 +46,9 @@ def lib():
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
+    L.bcf_find_buckets_workspace_bytes.restype = sz
+    L.bcf_find_buckets_workspace_bytes.argtypes = [sz, sz, ci, ci, ci, ci]
+    L.bcf_find_buckets.argtypes = [vp, sz, sz, ci, ci, ci, ci, vp, vp, vp, vp, sz, vp]
     L.bcf_set_rounds_per_pass.argtypes = [ci]
     L.bcf_merge_runs.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_runs_pagewise.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
@@ -207,6 +210,26 @@ def merge_pass_count(n, run_len, key_dtype=None, has_vals=False, kt=None, vt=Non
         kt = BCF_KEY_U64 if np.dtype(key_dtype).itemsize == 8 else BCF_KEY_U32
         vt = BCF_VAL_U32 if has_vals else BCF_VAL_NONE
     return int(lib().bcf_merge_pass_count(int(n), int(run_len), kt, vt))
+
+
+def find_buckets(keys, run_len, t, P, pivot_buckets=False, stream=None):
+    """bcf_find_buckets: returns (keys regrouped by bucket, pivots, piece_offsets[(nb*s + 1)])."""
+    torch = _torch()
+    kt, vt = _types(keys, None)
+    n = keys.numel()
+    s = -(-n // int(run_len))
+    nb = 2 * P - 1 if pivot_buckets else P
+    need = int(lib().bcf_find_buckets_workspace_bytes(n, int(run_len), int(t), int(P), int(bool(pivot_buckets)), kt))
+    if need == 0:
+        raise ValueError("find_buckets: invalid n / run_len / t / P")
+    ws = torch.empty(need, dtype=torch.uint8, device=keys.device)
+    out = torch.empty_like(keys)
+    pivots = torch.empty(P - 1, dtype=keys.dtype, device=keys.device)
+    offsets = torch.empty(nb * s + 1, dtype=torch.int32, device=keys.device)
+    _check(lib().bcf_find_buckets(_dev(keys, "keys"), n, int(run_len), int(t), int(P), int(bool(pivot_buckets)), kt,
+                                  out.data_ptr(), pivots.data_ptr(), offsets.data_ptr(), ws.data_ptr(), need,
+                                  _stream(stream)), "bcf_find_buckets")
+    return out, pivots, offsets
 
 
 def set_rounds_per_pass(rounds):

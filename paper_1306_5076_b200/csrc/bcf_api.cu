@@ -11,6 +11,7 @@
 #include "bcf_merge_pipe.cuh"
 #include "bcf_merge4.cuh"
 #include "bcf_long_tile.cuh"
+#include "bcf_buckets.cuh"
 #include <cstdlib>
 
 using namespace bcf;
@@ -699,6 +700,85 @@ bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, si
     BCF_DISPATCH(kt, vt, st = launch_partition4<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, n, run_len,
                                                    num_bounds, stream));
     return st;
+}
+
+// ------------------------------------------------------------------ FIND-BUCKETS (Alg. 7)
+
+static bool buckets_geom(size_t n, size_t run_len, int t, int P, int pivot_buckets, buckets::Geom *g)
+{
+    if (n == 0 || n >= (size_t(1) << 32) || run_len == 0 || t < 1 || P < 2) return false;
+    const size_t s = (n + run_len - 1) / run_len;
+    if (s > 65536 || (size_t)t > 65536 || (size_t)P > 65536 || s * (size_t)t < (size_t)P) return false;
+    g->n = n; g->run_len = run_len;
+    g->s = (unsigned)s; g->t = (unsigned)t; g->P = (unsigned)P;
+    g->pb = pivot_buckets ? 1 : 0;
+    g->nb = pivot_buckets ? 2u * P - 1u : (unsigned)P;
+    return (size_t)g->nb * s < (size_t(1) << 26);
+}
+
+size_t bcf_find_buckets_workspace_bytes(size_t n, size_t run_len, int t, int P, int pivot_buckets, bcf_key_t kt)
+{
+    buckets::Geom g;
+    if (!valid_types(kt, BCF_VAL_NONE) || !buckets_geom(n, run_len, t, P, pivot_buckets, &g)) return 0;
+    const size_t st = (size_t)g.s * g.t;
+    return align_up(st * key_bytes(kt), 256) + align_up((size_t)g.s * (g.nb + 1) * 4, 256) +
+           align_up(bcf_workspace_bytes(BCF_OP_SORT, st, 0, kt, BCF_VAL_NONE), 256) + 256;
+}
+
+bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int t, int P, int pivot_buckets, bcf_key_t kt,
+                            void *d_keys_out, void *d_pivots, uint32_t *d_piece_offsets, void *d_workspace,
+                            size_t workspace_bytes, bcf_stream_t stream)
+{
+    if (!valid_types(kt, BCF_VAL_NONE)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    buckets::Geom g;
+    if (!buckets_geom(n, run_len, t, P, pivot_buckets, &g)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_keys_out || !d_pivots || !d_piece_offsets || !d_workspace) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    const size_t kb = n * key_bytes(kt);
+    if (overlap(d_keys_in, kb, d_keys_out, kb)) return BCF_ERR_INVALID_ARG;
+    const size_t need = bcf_find_buckets_workspace_bytes(n, run_len, t, P, pivot_buckets, kt);
+    if (workspace_bytes < need) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    if (overlap(d_workspace, need, d_keys_in, kb) || overlap(d_workspace, need, d_keys_out, kb)) return BCF_ERR_INVALID_ARG;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    ProfileGroup profile_group(stream);
+
+    const size_t ns = (size_t)g.s * g.t;
+    char *ws = static_cast<char *>(d_workspace);
+    void *samples = ws;
+    uint32_t *bounds = reinterpret_cast<uint32_t *>(ws + align_up(ns * key_bytes(kt), 256));
+    char *sort_ws = reinterpret_cast<char *>(bounds) + align_up((size_t)g.s * (g.nb + 1) * 4, 256);
+    const size_t sort_ws_bytes = workspace_bytes - static_cast<size_t>(sort_ws - ws);
+    const bool k64 = (kt == BCF_KEY_U64);
+    {
+        const unsigned blocks = static_cast<unsigned>((ns + 255) / 256);
+        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
+        if (k64) buckets::sample_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, samples, g);
+        else buckets::sample_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, samples, g);
+    }
+    if (cudaPeekAtLastError() != cudaSuccess) return BCF_ERR_CUDA;
+    st = bcf_sort(samples, nullptr, ns, kt, BCF_VAL_NONE, sort_ws, sort_ws_bytes, stream);   // MERGESORT(S)
+    if (st != BCF_OK) return st;
+    {
+        const size_t work = (size_t)g.s * (g.P - 1);
+        const unsigned blocks = static_cast<unsigned>((work + 127) / 128);
+        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
+        if (k64) buckets::rank_kernel<2><<<blocks, 128, 0, stream>>>(d_keys_in, samples, d_pivots, bounds, g);
+        else buckets::rank_kernel<1><<<blocks, 128, 0, stream>>>(d_keys_in, samples, d_pivots, bounds, g);
+    }
+    {
+        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
+        buckets::offsets_kernel<<<1, buckets::SCAN_THREADS, 0, stream>>>(bounds, d_piece_offsets, g);
+    }
+    {
+        const size_t pieces = (size_t)g.nb * g.s;
+        const unsigned blocks = static_cast<unsigned>(pieces < 148 * 32 ? pieces : 148 * 32);
+        LaunchTimer tm(BCF_KERNEL_MERGE, stream);
+        if (k64) buckets::scatter_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
+        else buckets::scatter_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }
 
 bcf_status bcf_set_rounds_per_pass(int rounds)

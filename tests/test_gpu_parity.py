@@ -354,3 +354,31 @@ def test_kernels_use_no_local_memory(bcf):
                 info = bcf.kernel_info(cls, kt, vt)
                 assert info["local_bytes_per_thread"] == 0, (cls, kt, vt, info)
                 assert info["ctas_per_sm"] >= 1
+
+
+# ---------------------------------------------------------------- bcf_find_buckets
+
+
+@pytest.mark.parametrize("kind", ["u32", "u64"])
+@pytest.mark.parametrize("pb", [False, True])
+@pytest.mark.parametrize("n,run_len,t,P,dup", [
+    (64 * 1024, 4096, 16, 16, False), (64 * 1024, 4096, 16, 16, True), (100000, 7000, 5, 9, False),
+    (1 << 18, 1 << 12, 64, 64, True), (1 << 18, 1 << 14, 128, 128, False), (5000, 1024, 3, 2, True), (300, 100, 1, 3, False),
+])
+def test_find_buckets_matches_oracle(bcf, kind, pb, n, run_len, t, P, dup):
+    """Alg. 7 (and pivot buckets): pivots, piece offsets and the regrouped keys, exactly."""
+    keys, _ = make(kind, n, seed=n + t + P, dup=dup)
+    keys = workloads.sorted_runs(keys, run_len)
+    out, piv, off = bcf.find_buckets(dev(keys), run_len, t, P, pivot_buckets=pb)
+    O, F, Q = oracle.find_buckets(keys, run_len, t, P, pivot_buckets=pb)
+    assert np.array_equal(host(piv, keys), F)
+    assert np.array_equal(off.cpu().numpy().view(np.uint32).astype(np.int64), Q)
+    assert np.array_equal(host(out, keys), O)
+
+
+def test_find_buckets_pivot_buckets_sort_zero_one_data(bcf):
+    """0-1 data is sorted by the distribution alone when pivots get their own buckets."""
+    rng = np.random.default_rng(3)
+    keys = workloads.sorted_runs(rng.integers(0, 2, size=1 << 20).astype(np.uint32), 1 << 14)
+    out, _, _ = bcf.find_buckets(dev(keys), 1 << 14, 64, 64, pivot_buckets=True)
+    assert np.array_equal(host(out, keys), np.sort(keys))

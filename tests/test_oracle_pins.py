@@ -350,3 +350,65 @@ def test_corank_multi_equals_kway_merge_trace_and_two_way_corank():
     ka = [np.array([5, 5], np.uint32), np.array([5, 5], np.uint32)]
     va = [np.array([2, 9], np.uint32), np.array([1, 3], np.uint32)]
     assert [oracle.corank_multi(ka, d, va) for d in range(5)] == [[0, 0], [0, 1], [1, 1], [1, 2], [2, 2]]
+
+
+def _bucket_ranges(Q, s, nb):
+    return [(int(Q[b * s]), int(Q[(b + 1) * s])) for b in range(nb)]
+
+
+@pytest.mark.parametrize("pb", [False, True])
+def test_find_buckets_is_an_ordered_partition_and_meets_lemma_1(pb):
+    """Pins for oracle.find_buckets (section 3.2, Alg. 7): O is a permutation of the input,
+    every piece keeps its run's order, buckets are in ascending value order (so sorting each bucket gives
+    the sorted input), bucket contents match their definition by the pivots, and -- all keys distinct --
+    no bucket exceeds Lemma 1's bound s*ceil(N/(s t)) + ceil(s t / P)*ceil(N/(s t)) (L139-141)."""
+    rng = np.random.default_rng(5 + pb)
+    for trial in range(40):
+        s = int(rng.integers(2, 9)); run_len = int(rng.integers(8, 200)); t = int(rng.integers(1, 9))
+        P = int(rng.integers(2, min(s * t, 12) + 1))
+        n = s * run_len - int(rng.integers(0, run_len // 2))
+        distinct = trial % 2 == 0
+        if distinct:
+            keys = rng.permutation(1 << 16)[:n].astype(np.uint32)
+        else:
+            keys = rng.integers(0, 6, size=n).astype(np.uint32)
+        keys = workloads.sorted_runs(keys, run_len)
+        O, F, Q = oracle.find_buckets(keys, run_len, t, P, pivot_buckets=pb)
+        s_runs = -(-n // run_len)
+        nb = 2 * P - 1 if pb else P
+        assert np.array_equal(np.sort(O), np.sort(keys)) and Q[-1] == n and np.all(np.diff(Q) >= 0)
+        assert np.all(F[:-1] <= F[1:])
+        rngs = _bucket_ranges(Q, s_runs, nb)
+        for b, (lo, hi) in enumerate(rngs):
+            x = O[lo:hi]
+            if x.size == 0:
+                continue
+            if not pb:
+                if b > 0: assert x.min() > F[b - 1]
+                if b < P - 1: assert x.max() <= F[b]
+            elif b % 2 == 1:                                  # pivot bucket j = (b - 1) / 2: all equal to it
+                assert np.all(x == F[(b - 1) // 2])
+            else:
+                j = b // 2
+                if j > 0: assert x.min() > F[j - 1]
+                if j < P - 1: assert x.max() < F[j]
+            for r in range(s_runs):                           # pieces stay sorted
+                piece = O[Q[b * s_runs + r]:Q[b * s_runs + r + 1]]
+                assert np.all(piece[:-1] <= piece[1:])
+        sorted_by_bucket = np.concatenate([np.sort(O[lo:hi]) for lo, hi in rngs])
+        assert np.array_equal(sorted_by_bucket, np.sort(keys))
+        if distinct and not pb and n == s * run_len:
+            per = -(-n // (s * t))
+            bound = s * per + (-(-(s * t) // P)) * per
+            assert max(hi - lo for lo, hi in rngs) <= bound
+
+
+def test_find_buckets_pivot_buckets_finish_zero_one_data():
+    """on 0-1 data BCFMergesortPB "has nothing more to do after rearranging the data"."""
+    rng = np.random.default_rng(9)
+    keys = workloads.sorted_runs(rng.integers(0, 2, size=16 * 256).astype(np.uint32), 256)
+    O, F, Q = oracle.find_buckets(keys, 256, 8, 8, pivot_buckets=True)
+    assert np.array_equal(O, np.sort(keys))
+    s, nb = 16, 15
+    sizes = [int(Q[(b + 1) * s] - Q[b * s]) for b in range(nb)]
+    assert sum(sizes[1::2]) == keys.size and sum(sizes[0::2]) == 0     # every key sits in a pivot bucket
