@@ -319,6 +319,44 @@ def side_line(bcf, torch, dev, name, stream, barrier, variant=None):
         TILE_ALGO = saved[2]
 
 
+def buckets_line(bcf, torch, dev, stream, pivot_buckets, zero_one=False):
+    """bcf_find_buckets (Alg. 7; the paper's p = 128): 128 sorted runs totalling 2^27 uint32 keys,
+    t = P = 128.  Device-timed, 3 warm-ups, 5 steps (the call allocates nothing inside the timed region
+    except through torch's caching allocator, warmed up before)."""
+    n, k = 1 << 27, 128
+    if zero_one:
+        rng = np.random.Generator(np.random.Philox(key=workloads.seed_for(6, 1)))
+        keys = workloads.sorted_runs(rng.integers(0, 2, size=n, dtype=np.uint32), n // k)
+        run_len = n // k
+    else:
+        keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=n)
+    d = torch.from_numpy(keys.view(np.int32)).to(dev)
+    for _ in range(3):
+        out = bcf.find_buckets(d, run_len, k, k, pivot_buckets=pivot_buckets)
+    torch.cuda.synchronize()
+    sizes = out[2].cpu().numpy().view(np.uint32)[::k].astype(np.int64)
+    ms = []
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        out = bcf.find_buckets(d, run_len, k, k, pivot_buckets=pivot_buckets)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    t = sum(ms) / len(ms)
+    peak, _ = measured_peak()
+    line = {"workload": "find_buckets", "description": "FIND-BUCKETS (Alg. 7) of 128 sorted uint32 runs totalling 2^27 keys, "
+            "t = P = 128" + (", keys in {0, 1}" if zero_one else ", uniform keys"),
+            "variant": "pivot buckets" if pivot_buckets else "plain", "dtype": "u32", "n": n, "value": n / (t * 1e-3),
+            "unit": UNIT, "ms_per_step": t, "best_ms": min(ms), "passes": 1,
+            "frac_of_measured_hbm_peak_for_pass_count": 2 * 4 * n / (t * 1e-3) / 1e9 / peak,
+            "largest_bucket": int(np.diff(sizes).max()), "mean_bucket": n / (len(sizes) - 1),
+            "sorted_by_distribution_alone": bool((out[0][1:] >= out[0][:-1]).all().item()) if zero_one else None}
+    del d, out
+    torch.cuda.empty_cache()
+    return line
+
+
 def _side_line(bcf, torch, dev, name, stream, barrier, variant):
     desc, logn, gen, op, dtype = WORKLOADS[name]
     n = 1 << logn
@@ -522,6 +560,9 @@ def main():
                               {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
         side.append(side_line(bcf, torch, dev, "cfg2", stream, barrier,
                               {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
+        side.append(buckets_line(bcf, torch, dev, stream, False))
+        side.append(buckets_line(bcf, torch, dev, stream, True))
+        side.append(buckets_line(bcf, torch, dev, stream, True, zero_one=True))
 
     if rank == 0:
         print(json.dumps({

@@ -772,8 +772,8 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
         buckets::offsets_kernel<<<1, buckets::SCAN_THREADS, 0, stream>>>(bounds, d_piece_offsets, g);
     }
     {
-        const size_t pieces = (size_t)g.nb * g.s;
-        const unsigned blocks = static_cast<unsigned>(pieces < 148 * 32 ? pieces : 148 * 32);
+        const size_t chunks = ((run_len + buckets::SCATTER_CHUNK - 1) / buckets::SCATTER_CHUNK) * g.s;
+        const unsigned blocks = static_cast<unsigned>(chunks < 148 * 64 ? chunks : 148 * 64);
         LaunchTimer tm(BCF_KERNEL_MERGE, stream);
         if (k64) buckets::scatter_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
         else buckets::scatter_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);

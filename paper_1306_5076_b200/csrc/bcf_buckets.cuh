@@ -126,21 +126,39 @@ offsets_kernel(const uint32_t *__restrict__ bounds, uint32_t *__restrict__ Q, co
     if (threadIdx.x == SCAN_THREADS - 1) Q[total] = static_cast<uint32_t>(sums[SCAN_THREADS - 1]);
 }
 
-// O[Q[b s + r] ..] = piece (b, r): one CTA per piece, coalesced 4- or 8-byte copies.
+// O[Q[b s + r] ..] = piece (b, r).  One CTA per chunk of SCATTER_CHUNK consecutive elements of a run --
+// equal work for every CTA whatever the bucket sizes (0-1 data puts half of the input into one bucket):
+// the chunk's first bucket by binary search in the run's row of bounds, then bucket after bucket the
+// part of the chunk that falls into it is copied, coalesced, to its place in O.
+constexpr unsigned SCATTER_CHUNK = 8192;
 template <int KW>
 __global__ void __launch_bounds__(256)
 scatter_kernel(const void *__restrict__ kin, void *__restrict__ kout, const uint32_t *__restrict__ bounds,
                const uint32_t *__restrict__ Q, const Geom g)
 {
     using K = typename KeyT<KW>::type;
-    const unsigned long long total = static_cast<unsigned long long>(g.nb) * g.s;
+    const unsigned long long chunks_per_run = (g.run_len + SCATTER_CHUNK - 1) / SCATTER_CHUNK;
+    const unsigned long long total = chunks_per_run * g.s;
     for (unsigned long long e = blockIdx.x; e < total; e += gridDim.x) {
-        const unsigned int b = static_cast<unsigned int>(e / g.s), r = static_cast<unsigned int>(e % g.s);
+        const unsigned int r = static_cast<unsigned int>(e / chunks_per_run);
+        const unsigned long long len = run_length(g, r);
+        const unsigned long long c0 = (e % chunks_per_run) * SCATTER_CHUNK;
+        if (c0 >= len) continue;
+        const unsigned long long c1 = min(len, c0 + SCATTER_CHUNK);
         const uint32_t *row = bounds + static_cast<unsigned long long>(r) * (g.nb + 1);
-        const uint32_t from = row[b], len = row[b + 1] - from;
-        const K *src = static_cast<const K *>(kin) + static_cast<unsigned long long>(r) * g.run_len + from;
-        K *dst = static_cast<K *>(kout) + Q[e];
-        for (uint32_t i = threadIdx.x; i < len; i += blockDim.x) dst[i] = src[i];
+        unsigned int lo = 0, hi = g.nb;                      // last b with row[b] <= c0
+        while (lo + 1 < hi) {
+            const unsigned int mid = (lo + hi) >> 1;
+            if (row[mid] <= c0) lo = mid; else hi = mid;
+        }
+        const K *src = static_cast<const K *>(kin) + static_cast<unsigned long long>(r) * g.run_len;
+        for (unsigned int b = lo; b < g.nb && row[b] < c1; ++b) {
+            const unsigned long long from = max(c0, static_cast<unsigned long long>(row[b]));
+            const unsigned long long to = min(c1, static_cast<unsigned long long>(row[b + 1]));
+            if (from >= to) continue;
+            K *dst = static_cast<K *>(kout) + Q[static_cast<unsigned long long>(b) * g.s + r] - row[b];
+            for (unsigned long long i = from + threadIdx.x; i < to; i += blockDim.x) dst[i] = src[i];
+        }
     }
 }
 
