@@ -157,7 +157,13 @@ scatter_kernel(const void *__restrict__ kin, void *__restrict__ kout, const uint
             const unsigned long long to = min(c1, static_cast<unsigned long long>(row[b + 1]));
             if (from >= to) continue;
             K *dst = static_cast<K *>(kout) + Q[static_cast<unsigned long long>(b) * g.s + r] - row[b];
-            for (unsigned long long i = from + threadIdx.x; i < to; i += blockDim.x) dst[i] = src[i];
+            // four independent loads in flight per thread
+            unsigned long long i = from + threadIdx.x;
+            for (; i + 3 * 256 < to; i += 4 * 256) {
+                const K a = src[i], b2 = src[i + 256], c = src[i + 512], d = src[i + 768];
+                dst[i] = a; dst[i + 256] = b2; dst[i + 512] = c; dst[i + 768] = d;
+            }
+            for (; i < to; i += 256) dst[i] = src[i];
         }
     }
 }
