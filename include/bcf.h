@@ -195,6 +195,27 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
                             void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
 
 /*
+ * bcf_colored_prefix_sums -- conflict-free coloured prefix sums (Appendix A; SURVEY.md
+ * 8f item 4): d_out[i] = sum of d_values[j] over j <= i with d_colors[j] == d_colors[i], in uint32
+ * arithmetic (sums wrap modulo 2^32).  Three phases as in the paper (tile sums, exclusive scan of the
+ * tile sums per colour, page-wise scan of every tile); a thread's per-colour running sums are kept in
+ * shared memory.
+ *   d_values  : n uint32.   d_colors : n bytes, each < num_colors.   num_colors : 1..16.
+ *   layout    : BCF_SCAN_BANK_PER_THREAD -- word 32 c + lane, "one memory bank per thread" (L228): every
+ *               warp access hits 32 distinct banks whatever the colours;
+ *               BCF_SCAN_THREAD_MAJOR -- word d lane + c, the layout the paper starts from, kept to
+ *               reproduce its Figure 1 (bank conflicts and run time grow with d).  Same result.
+ *   d_out     : n uint32, may not overlap the inputs.
+ *   d_workspace : >= bcf_colored_prefix_sums_workspace_bytes(n) bytes.
+ * A colour >= num_colors is an unchecked precondition violation.
+ */
+typedef enum { BCF_SCAN_BANK_PER_THREAD = 0, BCF_SCAN_THREAD_MAJOR = 1 } bcf_scan_layout;
+size_t bcf_colored_prefix_sums_workspace_bytes(size_t n);
+bcf_status bcf_colored_prefix_sums(const uint32_t *d_values, const uint8_t *d_colors, size_t n, int num_colors,
+                                   int layout, uint32_t *d_out, void *d_workspace, size_t workspace_bytes,
+                                   bcf_stream_t stream);
+
+/*
  * Number of passes over global memory (one read + one write of all n elements each) that
  * bcf_merge_runs takes from runs of run_len: a pass does two merge rounds where the four-run
  * kernel applies (run_len = 1024 * 2^k and the element type's stage buffers fit one SM) and one

@@ -217,3 +217,24 @@ def find_buckets(keys, run_len, t, P, pivot_buckets=False):
             oc += piece.size
     Q[nb * s] = oc
     return O, F, Q
+
+
+def colored_prefix_sums(values, colors, num_colors):
+    """Coloured prefix sums (Appendix A): "given an array of N elements and a set of d
+    colors, with a color associated with each element, compute d independent prefix sums among the
+    elements of the same color".  The definition written out, one element after the other:
+    out[i] = sum of values[j], j <= i, colors[j] == colors[i] (inclusive), uint32 arithmetic."""
+    v = np.ascontiguousarray(values, dtype=np.uint32)
+    c = np.ascontiguousarray(colors, dtype=np.uint8)
+    if v.shape != c.shape or (c.size and int(c.max()) >= num_colors):
+        raise ValueError("bad colours")
+    running = [0] * num_colors
+    out = np.empty_like(v)
+    vi, ci = v.tolist(), c.tolist()
+    res = [0] * len(vi)
+    for i in range(len(vi)):
+        k = ci[i]
+        running[k] = (running[k] + vi[i]) & 0xFFFFFFFF
+        res[i] = running[k]
+    out[:] = np.array(res, dtype=np.uint32) if res else out
+    return out

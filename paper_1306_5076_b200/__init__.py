@@ -18,6 +18,9 @@ from .binding import (  # noqa: F401
     layout_access,
     layout_word,
     lib,
+    colored_prefix_sums,
+    SCAN_BANK_PER_THREAD,
+    SCAN_THREAD_MAJOR,
     find_buckets,
     merge_partition,
     merge_partition4,

@@ -46,6 +46,9 @@ def lib():
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
+    L.bcf_colored_prefix_sums_workspace_bytes.restype = sz
+    L.bcf_colored_prefix_sums_workspace_bytes.argtypes = [sz]
+    L.bcf_colored_prefix_sums.argtypes = [vp, vp, sz, ci, ci, vp, vp, sz, vp]
     L.bcf_find_buckets_workspace_bytes.restype = sz
     L.bcf_find_buckets_workspace_bytes.argtypes = [sz, sz, ci, ci, ci, ci]
     L.bcf_find_buckets.argtypes = [vp, sz, sz, ci, ci, ci, ci, vp, vp, vp, vp, sz, vp]
@@ -230,6 +233,28 @@ def find_buckets(keys, run_len, t, P, pivot_buckets=False, stream=None):
                                   out.data_ptr(), pivots.data_ptr(), offsets.data_ptr(), ws.data_ptr(), need,
                                   _stream(stream)), "bcf_find_buckets")
     return out, pivots, offsets
+
+
+SCAN_BANK_PER_THREAD, SCAN_THREAD_MAJOR = 0, 1
+
+
+def colored_prefix_sums(values, colors, num_colors, layout=SCAN_BANK_PER_THREAD, out=None, workspace=None, stream=None):
+    """bcf_colored_prefix_sums: values int32/uint32 tensor, colors uint8 tensor (< num_colors) -> out."""
+    torch = _torch()
+    if values.dtype not in (torch.int32, torch.uint32) or colors.dtype != torch.uint8:
+        raise TypeError("values must be a 32-bit integer tensor and colors a uint8 tensor")
+    n = values.numel()
+    if colors.numel() != n:
+        raise ValueError("values and colors must have the same number of elements")
+    if out is None:
+        out = torch.empty_like(values)
+    need = int(lib().bcf_colored_prefix_sums_workspace_bytes(n))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=values.device)
+    _check(lib().bcf_colored_prefix_sums(_dev(values, "values"), _dev(colors, "colors"), n, int(num_colors), int(layout),
+                                         _dev(out, "out"), workspace.data_ptr(), workspace.numel(), _stream(stream)),
+           "bcf_colored_prefix_sums")
+    return out
 
 
 def set_rounds_per_pass(rounds):

@@ -12,6 +12,7 @@
 #include "bcf_merge4.cuh"
 #include "bcf_long_tile.cuh"
 #include "bcf_buckets.cuh"
+#include "bcf_colored_scan.cuh"
 #include <cstdlib>
 
 using namespace bcf;
@@ -777,6 +778,54 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
         LaunchTimer tm(BCF_KERNEL_MERGE, stream);
         if (k64) buckets::scatter_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
         else buckets::scatter_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
+    }
+    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------ coloured prefix sums (App. A)
+
+static unsigned colored_scan_grid(size_t n)
+{
+    const size_t pages = (n + cscan::PAGE - 1) / cscan::PAGE;
+    const size_t ctas = (pages + cscan::WARPS - 1) / cscan::WARPS;
+    return static_cast<unsigned>(ctas < 2048 ? ctas : 2048);
+}
+
+size_t bcf_colored_prefix_sums_workspace_bytes(size_t n)
+{
+    if (n == 0) return 0;
+    return align_up(size_t(colored_scan_grid(n)) * cscan::WARPS * cscan::MAX_COLORS * 4, 256);
+}
+
+bcf_status bcf_colored_prefix_sums(const uint32_t *d_values, const uint8_t *d_colors, size_t n, int num_colors, int layout,
+                                   uint32_t *d_out, void *d_workspace, size_t workspace_bytes, bcf_stream_t stream)
+{
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || num_colors < 1 || num_colors > cscan::MAX_COLORS) return BCF_ERR_INVALID_ARG;
+    if (layout != BCF_SCAN_BANK_PER_THREAD && layout != BCF_SCAN_THREAD_MAJOR) return BCF_ERR_INVALID_ARG;
+    if (!d_values || !d_colors || !d_out || !d_workspace) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_values) || !aligned16(d_colors) || !aligned16(d_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    if (workspace_bytes < bcf_colored_prefix_sums_workspace_bytes(n)) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    bcf_status st = check_device();
+    if (st != BCF_OK) return st;
+    ProfileGroup profile_group(stream);
+    const unsigned grid = colored_scan_grid(n);
+    const unsigned long long warps = static_cast<unsigned long long>(grid) * cscan::WARPS;
+    uint32_t *partial = static_cast<uint32_t *>(d_workspace);
+    const bool cf = (layout == BCF_SCAN_BANK_PER_THREAD);
+    {
+        LaunchTimer t(BCF_KERNEL_PARTITION, stream);
+        if (cf) cscan::reduce_kernel<true><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial);
+        else cscan::reduce_kernel<false><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial);
+    }
+    {
+        LaunchTimer t(BCF_KERNEL_PARTITION, stream);
+        cscan::offsets_kernel<<<1, cscan::MAX_COLORS * 32, 0, stream>>>(partial, warps, num_colors);
+    }
+    {
+        LaunchTimer t(BCF_KERNEL_MERGE, stream);
+        if (cf) cscan::scan_kernel<true><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial, d_out);
+        else cscan::scan_kernel<false><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial, d_out);
     }
     return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
 }

@@ -382,3 +382,20 @@ def test_find_buckets_pivot_buckets_sort_zero_one_data(bcf):
     keys = workloads.sorted_runs(rng.integers(0, 2, size=1 << 20).astype(np.uint32), 1 << 14)
     out, _, _ = bcf.find_buckets(dev(keys), 1 << 14, 64, 64, pivot_buckets=True)
     assert np.array_equal(host(out, keys), np.sort(keys))
+
+
+# ---------------------------------------------------------------- bcf_colored_prefix_sums
+
+
+@pytest.mark.parametrize("layout", [0, 1], ids=["bank_per_thread", "thread_major"])
+@pytest.mark.parametrize("n,d", [(1, 1), (15, 3), (511, 16), (512, 2), (513, 7), (4096 * 3 + 5, 16), (100000, 1),
+                                 (1 << 20, 16), ((1 << 20) + 12345, 5), ((1 << 23) + 3, 11)])
+def test_colored_prefix_sums_match_oracle(bcf, layout, n, d):
+    """App. A: every output element, both shared-memory layouts, ragged sizes, 1..16 colours."""
+    rng = np.random.default_rng(n + d)
+    vals = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(np.uint32)
+    cols = rng.integers(0, d, size=n).astype(np.uint8)
+    if n > 2000:
+        cols[100:1500] = d - 1                      # a long single-colour stretch
+    out = bcf.colored_prefix_sums(dev(vals), torch.from_numpy(cols).cuda(), d, layout=layout)
+    assert np.array_equal(host(out, vals), oracle.colored_prefix_sums(vals, cols, d))

@@ -412,3 +412,23 @@ def test_find_buckets_pivot_buckets_finish_zero_one_data():
     s, nb = 16, 15
     sizes = [int(Q[(b + 1) * s] - Q[b * s]) for b in range(nb)]
     assert sum(sizes[1::2]) == keys.size and sum(sizes[0::2]) == 0     # every key sits in a pivot bucket
+
+
+def test_colored_prefix_sums_pins():
+    """oracle.colored_prefix_sums (PAPER.md App. A): one colour = the textbook inclusive scan (numpy cumsum);
+    d colours = the scan of each colour's subsequence, put back in place; the last element of every colour
+    carries that colour's total; wrap-around modulo 2^32."""
+    rng = np.random.default_rng(21)
+    v = rng.integers(0, 1 << 32, size=5000, dtype=np.uint64).astype(np.uint32)
+    one = oracle.colored_prefix_sums(v, np.zeros(v.size, np.uint8), 1)
+    assert np.array_equal(one, np.cumsum(v.astype(np.uint64)).astype(np.uint32))      # mod 2^32 by truncation
+    for d in (2, 3, 16):
+        c = rng.integers(0, d, size=v.size).astype(np.uint8)
+        out = oracle.colored_prefix_sums(v, c, d)
+        for k in range(d):
+            m = c == k
+            assert np.array_equal(out[m], np.cumsum(v[m].astype(np.uint64)).astype(np.uint32))
+            if m.any():
+                assert int(out[np.flatnonzero(m)[-1]]) == int(v[m].astype(np.uint64).sum() & 0xFFFFFFFF)
+    assert oracle.colored_prefix_sums(np.array([1, 2, 3, 4], np.uint32), np.array([0, 1, 0, 1], np.uint8), 2).tolist() == [1, 2, 4, 6]
+    assert oracle.colored_prefix_sums(np.array([0xFFFFFFFF, 2], np.uint32), np.array([0, 0], np.uint8), 1).tolist() == [0xFFFFFFFF, 1]
