@@ -357,6 +357,43 @@ def buckets_line(bcf, torch, dev, stream, pivot_buckets, zero_one=False):
     return line
 
 
+def colored_scan_lines(bcf, torch, dev, stream):
+    """bcf_colored_prefix_sums (App. A, Figure 1): 2^28 uint32 values, colours i.i.d. uniform over d,
+    for d = 1, 4, 16 and both shared-memory layouts.  Device-timed, 2 warm-ups, 5 steps each.
+    Algorithmic bytes: phase 1 reads 5 n, phase 3 reads 5 n and writes 4 n = 14 n."""
+    n = 1 << 28
+    g = torch.Generator(device=dev)
+    g.manual_seed(workloads.seed_for(7, 0))
+    vals = torch.randint(-2 ** 31, 2 ** 31 - 1, (n,), dtype=torch.int32, device=dev, generator=g)
+    out = torch.empty_like(vals)
+    ws = torch.empty(1 << 21, dtype=torch.uint8, device=dev)
+    peak, _ = measured_peak()
+    lines = []
+    for d in (1, 4, 16):
+        cols = torch.randint(0, d, (n,), dtype=torch.uint8, device=dev, generator=g)
+        for layout, lname in ((bcf.SCAN_BANK_PER_THREAD, "bank per thread (conflict-free)"),
+                              (bcf.SCAN_THREAD_MAJOR, "thread-major (the layout the paper starts from)")):
+            for _ in range(2):
+                bcf.colored_prefix_sums(vals, cols, d, layout=layout, out=out, workspace=ws)
+            ms = []
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                bcf.colored_prefix_sums(vals, cols, d, layout=layout, out=out, workspace=ws)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+            t = sum(ms) / len(ms)
+            lines.append({"workload": "colored_prefix_sums", "description": "coloured prefix sums of 2^28 uint32 values, "
+                          "%d colours (PAPER.md App. A)" % d, "variant": lname, "dtype": "u32", "n": n, "colors": d,
+                          "value": n / (t * 1e-3), "unit": "elements/s", "ms_per_step": t, "best_ms": min(ms), "passes": 2,
+                          "frac_of_measured_hbm_peak_for_pass_count": 14 * n / (t * 1e-3) / 1e9 / peak})
+        del cols
+    del vals, out, ws
+    torch.cuda.empty_cache()
+    return lines
+
+
 def _side_line(bcf, torch, dev, name, stream, barrier, variant):
     desc, logn, gen, op, dtype = WORKLOADS[name]
     n = 1 << logn
@@ -563,6 +600,7 @@ def main():
         side.append(buckets_line(bcf, torch, dev, stream, False))
         side.append(buckets_line(bcf, torch, dev, stream, True))
         side.append(buckets_line(bcf, torch, dev, stream, True, zero_one=True))
+        side.extend(colored_scan_lines(bcf, torch, dev, stream))
 
     if rank == 0:
         print(json.dumps({

@@ -21,7 +21,15 @@
 namespace bcf {
 namespace cscan {
 
-constexpr int CH = 16;                 // elements per lane per page (one 16-byte load of colours)
+#ifndef BCF_CSCAN_CH
+#define BCF_CSCAN_CH 16
+#endif
+// A lane reads its chunk with 16-byte loads 64 bytes apart: the two halves of a 32-byte sector arrive in
+// two different instructions, so these loads DO allocate in L1 (unlike the streaming loads of the sort).
+#ifndef BCF_CSCAN_LD
+#define BCF_CSCAN_LD(p) __ldg(p)
+#endif
+constexpr int CH = BCF_CSCAN_CH;       // elements per lane per page (a multiple of 16: 16-byte loads of colours)
 constexpr int PAGE = 32 * CH;          // elements per warp per page
 constexpr int WARPS = 8;               // warps per CTA
 constexpr int MAX_COLORS = 16;
@@ -53,7 +61,7 @@ __device__ __forceinline__ void warp_pages(const unsigned long long n, const uns
     last = min(pages, first + per);
 }
 
-// this lane's chunk of a page: 16 values and 16 colours (missing elements: value 0, colour 0)
+// this lane's chunk of a page: CH values and CH colours (missing elements: value 0, colour 0)
 __device__ __forceinline__ void load_chunk(const uint32_t *__restrict__ vals, const unsigned char *__restrict__ cols,
                                            const unsigned long long base, const unsigned long long n, uint32_t (&v)[CH],
                                            uint32_t (&c)[CH])
@@ -62,13 +70,16 @@ __device__ __forceinline__ void load_chunk(const uint32_t *__restrict__ vals, co
         const uint4 *pv = reinterpret_cast<const uint4 *>(vals + base);
 #pragma unroll
         for (int q = 0; q < CH / 4; ++q) {
-            const uint4 t = ldg128(pv + q);
+            const uint4 t = BCF_CSCAN_LD(pv + q);
             v[4 * q] = t.x; v[4 * q + 1] = t.y; v[4 * q + 2] = t.z; v[4 * q + 3] = t.w;
         }
-        const uint4 t = ldg128(reinterpret_cast<const uint4 *>(cols + base));
-        const uint32_t w[4] = {t.x, t.y, t.z, t.w};
 #pragma unroll
-        for (int k = 0; k < CH; ++k) c[k] = (w[k / 4] >> (8 * (k % 4))) & 0xFFu;
+        for (int q = 0; q < CH / 16; ++q) {
+            const uint4 t = BCF_CSCAN_LD(reinterpret_cast<const uint4 *>(cols + base) + q);
+            const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+            for (int k = 0; k < 16; ++k) c[16 * q + k] = (w[k / 4] >> (8 * (k % 4))) & 0xFFu;
+        }
     } else {
 #pragma unroll
         for (int k = 0; k < CH; ++k) {
