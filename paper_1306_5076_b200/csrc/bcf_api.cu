@@ -805,6 +805,7 @@ bcf_status bcf_colored_prefix_sums(const uint32_t *d_values, const uint8_t *d_co
     if (layout != BCF_SCAN_BANK_PER_THREAD && layout != BCF_SCAN_THREAD_MAJOR) return BCF_ERR_INVALID_ARG;
     if (!d_values || !d_colors || !d_out || !d_workspace) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_values) || !aligned16(d_colors) || !aligned16(d_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    if (overlap(d_out, n * 4, d_values, n * 4) || overlap(d_out, n * 4, d_colors, n)) return BCF_ERR_INVALID_ARG;
     if (workspace_bytes < bcf_colored_prefix_sums_workspace_bytes(n)) return BCF_ERR_WORKSPACE_TOO_SMALL;
     bcf_status st = check_device();
     if (st != BCF_OK) return st;

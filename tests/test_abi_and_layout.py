@@ -206,3 +206,43 @@ def test_tile_mergesort_column_sweep_reads_P_then_reversed_Q():
             for lane in range(32):
                 w, width = bcf.layout_access(8, 32 * (T - 1) + k, lane)
                 assert width == 1 and where[w] == seq[32 * (k - base) + lane]
+
+
+def test_argument_errors_are_reported_before_any_device_work():
+    """Status codes for bad arguments come back on a box without a GPU too (include/bcf.h, ERRORS)."""
+    L = bcf.lib()
+    INVALID, MISALIGNED, TOO_SMALL = 1, 2, 3
+    buf = np.zeros(1 << 16, dtype=np.uint8)
+    p = (buf.ctypes.data + 255) & ~255
+    assert L.bcf_set_base_case(7) == INVALID and L.bcf_set_rounds_per_pass(3) == INVALID
+    assert L.bcf_set_base_case(3) == 0 and L.bcf_get_base_case() == 3
+    assert L.bcf_set_rounds_per_pass(1) == 0 and L.bcf_get_rounds_per_pass() == 1
+    assert L.bcf_sort_long_tiles(p, None, 1, 3, 0, 0, None) == INVALID                 # h must be 2, 4 or 8
+    assert L.bcf_sort_long_tiles(p + 4, None, 1, 2, 0, 0, None) == MISALIGNED
+    assert L.bcf_sort_tiles_mergesort(None, None, 1, 0, 0, None) == INVALID
+    assert L.bcf_sort_tiles_mergesort(p, None, 0, 0, 0, None) == 0                      # nothing to do
+    # FIND-BUCKETS: P >= 2, s * t >= P, workspace
+    assert L.bcf_find_buckets_workspace_bytes(4096, 1024, 4, 1, 0, 0) == 0
+    assert L.bcf_find_buckets_workspace_bytes(4096, 1024, 1, 8, 0, 0) == 0              # 4 samples, 8 buckets
+    need = L.bcf_find_buckets_workspace_bytes(4096, 1024, 4, 8, 1, 0)
+    assert need > 0
+    assert L.bcf_find_buckets(p, 4096, 1024, 4, 1, 0, 0, p + 16384, p + 40000, p + 44000, p + 48000, need, None) == INVALID
+    assert L.bcf_find_buckets(p, 4096, 1024, 4, 8, 0, 0, p + 16384, p + 40000, p + 44000, p + 48000, 16, None) == TOO_SMALL
+    assert L.bcf_find_buckets(p, 4096, 1024, 4, 8, 0, 0, p + 1024, p + 40000, p + 44000, p + 48000, need, None) == INVALID  # in/out overlap
+    # coloured prefix sums: 1..16 colours, known layout, no aliasing
+    assert L.bcf_colored_prefix_sums_workspace_bytes(0) == 0 and L.bcf_colored_prefix_sums_workspace_bytes(1000) > 0
+    ws = L.bcf_colored_prefix_sums_workspace_bytes(1000)
+    assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 17, 0, p + 16384, p + 32768, ws, None) == INVALID
+    assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 0, 0, p + 16384, p + 32768, ws, None) == INVALID
+    assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 4, 2, p + 16384, p + 32768, ws, None) == INVALID
+    assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 4, 0, p, p + 32768, ws, None) == INVALID          # out aliases values
+    assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 4, 0, p + 16384, p + 32768, 0, None) == TOO_SMALL
+    # pass structure of the merging phase (host only)
+    assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0) == 18 and L.bcf_merge_pass_count(1 << 28, 8192, 0, 0) == 15
+    assert L.bcf_set_rounds_per_pass(2) == 0
+    try:
+        assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0) == 9
+        assert L.bcf_merge_pass_count(1 << 27, 1024, 0, 0) == 9     # 17 rounds: one two-way pass + 8 four-run passes
+        assert L.bcf_merge_pass_count(1 << 26, 1024, 1, 1) == 16    # (u64,u32): the four-run stage buffers do not fit
+    finally:
+        L.bcf_set_rounds_per_pass(1)
