@@ -15,7 +15,6 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC",
-    "--split-compile", "0",          # optimise the kernels of the one translation unit on all host cores
 ]
 
 
