@@ -173,7 +173,21 @@ def corank_multi(runs_keys, d, runs_vals=None):
     return [int(np.count_nonzero((first >= bounds[r]) & (first < bounds[r + 1]))) for r in range(len(ks))]
 
 
-def find_buckets(keys, run_len, t, P, pivot_buckets=False):
+def alg7_sample_index(i, length, t):
+    """Position of potential splitter i (0 <= i < t) in a sorted run of `length` elements.
+    PAPER.md Alg. 7: "S[pid t + i] = I_pid[i n/t]" -> floor(i length / t): the first sample is the
+    run's first element.  Pinned by tests/golden/alg7_worked_example.txt (S_UNSORTED)."""
+    return (i * length) // t
+
+
+def alg7_pivot_index(j, s, t, P):
+    """Position in the sorted sample array S (s t entries) of final pivot j (0 <= j < P - 1).
+    PAPER.md L135 "P-1 evenly spaced items from S", Alg. 7 "every t-th element of S" (s = P runs):
+    S[t], S[2t], .. = S[floor((j+1) s t / P)].  Pinned by tests/golden/alg7_worked_example.txt (F)."""
+    return ((j + 1) * s * t) // P
+
+
+def find_buckets(keys, run_len, t, P, pivot_buckets=False, return_steps=False):
     """FIND-BUCKETS, section 3.2 "Distribution" (L131-137) / Algorithm 7 (L492-520), with the
     pivot buckets of L155 as an option; reading A18 of DESIGN.md for the garbled lines.  Step by step:
       1. S: t samples of each of the s sorted runs, sample i of run r = its element floor(i len_r / t)
@@ -184,15 +198,16 @@ def find_buckets(keys, run_len, t, P, pivot_buckets=False):
          I[i] > F[c]); with pivot buckets also the number of elements < pivot;
       5. bucket sizes summed over the runs, exclusive prefix sums (L512-513);
       6. O = the runs' pieces regrouped by bucket, inside a bucket by run (L515-520).
-    Keys only.  Returns (O, F, Q) with Q[b s + r] = start of piece (bucket b, run r) in O, Q[-1] = n."""
+    Keys only.  Returns (O, F, Q) with Q[b s + r] = start of piece (bucket b, run r) in O, Q[-1] = n;
+    with return_steps also a dict of the intermediate arrays (S unsorted, S sorted, ranks) the golden pins."""
     k = np.ascontiguousarray(keys)
     _suffix(k)
     n = k.size
     s = -(-n // run_len)
     runs = [k[r * run_len:min(n, (r + 1) * run_len)] for r in range(s)]
-    S = np.array([run[(i * run.size) // t] for run in runs for i in range(t)], dtype=k.dtype)
-    S = np.sort(S, kind="stable")
-    F = np.array([S[((j + 1) * s * t) // P] for j in range(P - 1)], dtype=k.dtype)
+    S_unsorted = np.array([run[alg7_sample_index(i, run.size, t)] for run in runs for i in range(t)], dtype=k.dtype)
+    S = np.sort(S_unsorted, kind="stable")
+    F = np.array([S[alg7_pivot_index(j, s, t, P)] for j in range(P - 1)], dtype=k.dtype)
     nb = 2 * P - 1 if pivot_buckets else P
     bounds = np.zeros((s, nb + 1), dtype=np.int64)
     for r, run in enumerate(runs):
@@ -216,7 +231,95 @@ def find_buckets(keys, run_len, t, P, pivot_buckets=False):
             O[oc:oc + piece.size] = piece
             oc += piece.size
     Q[nb * s] = oc
+    if return_steps:
+        rank_le = np.array([[int(np.searchsorted(run, f, side="right")) for run in runs] for f in F], dtype=np.int64)
+        return O, F, Q, {"S_unsorted": S_unsorted, "S_sorted": S, "rank_le": rank_le.reshape(P - 1, s)}
     return O, F, Q
+
+
+def base_case_runs(keys, w=32):
+    """Base case phase alone (section 3, App. B): every tile of w*w keys ShearSorted, a last
+    partial tile padded with the maximum key (L420) and cut back.  Returns the array of sorted runs of w*w."""
+    k = np.ascontiguousarray(keys)
+    M = w * w
+    out = np.empty_like(k)
+    full = (k.size // M) * M
+    if full:
+        out[:full] = shearsort_tiles(k[:full], w=w)
+    if full < k.size:
+        pad = np.full(M, np.iinfo(k.dtype).max, dtype=k.dtype)
+        pad[:k.size - full] = k[full:]
+        out[full:] = shearsort_tiles(pad, w=w)[:k.size - full]
+    return out
+
+
+def merge_round(keys, run_len):
+    """ONE round of pairwise merging: runs 2p, 2p+1 of run_len -> one run of 2 run_len,
+    two-finger merge (L125); an odd last run is copied through."""
+    k = np.ascontiguousarray(keys)
+    out = np.empty_like(k)
+    for a0 in range(0, k.size, 2 * run_len):
+        a1 = min(k.size, a0 + run_len)
+        b1 = min(k.size, a1 + run_len)
+        out[a0:b1] = merge_two(k[a0:a1], k[a1:b1]) if b1 > a1 else k[a0:a1]
+    return out
+
+
+def merge_pieces(pieces):
+    """Final merge phase inside ONE bucket (section 3.2 "Final merge phase" L141-143, App. B):
+    the bucket's sorted subsequences (one per run, any lengths, possibly empty) merged pairwise in
+    ceil(log2 s) rounds of two-finger merges; a piece without a partner is carried to the next round.
+    Returns (sorted bucket, rounds)."""
+    cur = [np.ascontiguousarray(p) for p in pieces]
+    rounds = 0
+    while len(cur) > 1:
+        cur = [merge_two(cur[i], cur[i + 1]) if i + 1 < len(cur) else cur[i] for i in range(0, len(cur), 2)]
+        rounds += 1
+    return (cur[0] if cur else np.empty(0, dtype=np.uint32)), rounds
+
+
+def sort_full_buckets(keys, P, t=None, pivot_buckets=False, w=32, return_info=False):
+    """BCFMergesort with the paper's bucket distribution, end to end (BCFMergesortPB when pivot_buckets):
+    PAPER.md section 3.2 and App. B, the four phases in the paper's order:
+      1. base case: tiles of M = w*w keys ShearSorted (L103, L236);
+      2. first merge phase: rounds of pairwise merging while more than P runs remain -- "we suspend the
+         merge at s = P" (L131; for run counts that are not P * 2^k: at the first s <= P);
+      3. bucket distribution: FIND-BUCKETS on the s runs with t samples per run (default t = P, L139) and
+         P buckets (2P-1 with pivot buckets, L155) -- find_buckets above;
+      4. final merge phase: "CTA p_i then sorts the i-th bucket by merging the sorted subsequences of the
+         bucket" (L141), ceil(log2 s) rounds inside every bucket (L143); a pivot bucket holds copies of one
+         key and is already final (L155).
+    A single run after phase 2 (s = 1) is the result.  Keys only.  With return_info also a dict: runs s at the
+    distribution, run length, rounds of both merge phases, bucket sizes."""
+    k = np.ascontiguousarray(keys)
+    _suffix(k)
+    n, M = k.size, w * w
+    t = P if t is None else t
+    cur = base_case_runs(k, w)
+    run_len, rounds1 = M, 0
+    while -(-n // run_len) > P:
+        cur = merge_round(cur, run_len)
+        run_len *= 2
+        rounds1 += 1
+    s = -(-n // run_len) if n else 0
+    info = {"s": s, "run_len": run_len, "first_phase_rounds": rounds1, "final_phase_rounds": 0, "bucket_sizes": []}
+    if s <= 1:
+        return (cur, info) if return_info else cur
+    O, F, Q = find_buckets(cur, run_len, t, P, pivot_buckets=pivot_buckets)
+    nb = 2 * P - 1 if pivot_buckets else P
+    out = np.empty_like(k)
+    for b in range(nb):
+        lo, hi = int(Q[b * s]), int(Q[(b + 1) * s])
+        info["bucket_sizes"].append(hi - lo)
+        if hi == lo:
+            continue                                    # an empty bucket has nothing to merge
+        if pivot_buckets and b % 2 == 1:
+            out[lo:hi] = O[lo:hi]                       # copies of pivot (b-1)/2: already in final position
+            continue
+        merged, r = merge_pieces([O[int(Q[b * s + i]):int(Q[b * s + i + 1])] for i in range(s)])
+        out[lo:hi] = merged
+        info["final_phase_rounds"] = max(info["final_phase_rounds"], r)
+    return (out, info) if return_info else out
 
 
 def colored_prefix_sums(values, colors, num_colors):

@@ -432,3 +432,139 @@ def test_colored_prefix_sums_pins():
                 assert int(out[np.flatnonzero(m)[-1]]) == int(v[m].astype(np.uint64).sum() & 0xFFFFFFFF)
     assert oracle.colored_prefix_sums(np.array([1, 2, 3, 4], np.uint32), np.array([0, 1, 0, 1], np.uint8), 2).tolist() == [1, 2, 4, 6]
     assert oracle.colored_prefix_sums(np.array([0xFFFFFFFF, 2], np.uint32), np.array([0, 0], np.uint8), 1).tolist() == [0xFFFFFFFF, 1]
+
+
+# ---------------------------------------------------------------- Alg. 7 golden (hand-worked) and mutation pins
+
+
+def _load_alg7_golden():
+    """tests/golden/alg7_worked_example.txt -> list of dicts (every number in it was worked by hand from
+    PAPER.md L133-135, Alg. 7 L503-520 and L155; see the file header)."""
+    cases, cur = [], None
+    with open(os.path.join(os.path.dirname(__file__), "golden", "alg7_worked_example.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            key, *rest = line.split()
+            if key == "CASE":
+                cur = {"name": rest[0], "RANK_LE": []}
+            elif key == "END":
+                cases.append(cur)
+                cur = None
+            elif key == "RANK_LE":
+                cur["RANK_LE"].append([int(x) for x in rest])
+            elif key in ("RUN_LEN", "T", "P", "PIVOT_BUCKETS"):
+                cur[key] = int(rest[0])
+            else:
+                cur[key] = [int(x) for x in rest]
+    assert len(cases) == 4
+    return cases
+
+
+def _alg7_matches_golden(c, dtype=np.uint32):
+    O, F, Q, steps = oracle.find_buckets(np.array(c["I"], dtype=dtype), c["RUN_LEN"], c["T"], c["P"],
+                                         pivot_buckets=bool(c["PIVOT_BUCKETS"]), return_steps=True)
+    return (steps["S_unsorted"].tolist() == c["S_UNSORTED"] and steps["S_sorted"].tolist() == c["S_SORTED"]
+            and F.tolist() == c["F"] and steps["rank_le"].tolist() == c["RANK_LE"]
+            and O.tolist() == c["O"] and Q.tolist() == c["Q"])
+
+
+@pytest.mark.parametrize("dtype", [np.uint32, np.uint64])
+def test_find_buckets_reproduces_the_hand_worked_alg7_examples(dtype):
+    """oracle.find_buckets step by step against tests/golden/alg7_worked_example.txt: samples (L503),
+    sorted samples (L505), pivots (L506, L135), ranks (L507-510), regrouped output and offsets (L512-520),
+    with a ragged last run, a repeated pivot, and pivot buckets (L155)."""
+    for c in _load_alg7_golden():
+        assert _alg7_matches_golden(c, dtype), c["name"]
+
+
+@pytest.mark.parametrize("mutant", ["pivot_j_instead_of_j_plus_1", "pivot_minus_1", "sample_last_of_each_stride"])
+def test_alg7_golden_rejects_plausible_misreadings(monkeypatch, mutant):
+    """Mutation pins: each plausible misreading of Alg. 7's two index formulas (pivot j at S[j s t / P], at
+    S[(j+1) s t / P - 1], sample i at floor((i+1) len / t) - 1) must make the golden comparison fail -- the
+    Lemma 1 bound and the partition properties alone do not see them."""
+    if mutant == "pivot_j_instead_of_j_plus_1":
+        monkeypatch.setattr(oracle, "alg7_pivot_index", lambda j, s, t, P: (j * s * t) // P)
+    elif mutant == "pivot_minus_1":
+        monkeypatch.setattr(oracle, "alg7_pivot_index", lambda j, s, t, P: ((j + 1) * s * t) // P - 1)
+    else:
+        monkeypatch.setattr(oracle, "alg7_sample_index", lambda i, length, t: ((i + 1) * length) // t - 1)
+    results = [_alg7_matches_golden(c) for c in _load_alg7_golden()]
+    assert not all(results), (mutant, results)
+    assert not results[0], "the distinct-key example alone must catch the mutant"
+
+
+# ---------------------------------------------------------------- BCFMergesort with buckets, end to end
+
+
+def _ceil_log2(x):
+    return max(0, int(math.ceil(math.log2(x)))) if x > 1 else 0
+
+
+@pytest.mark.parametrize("pb", [False, True])
+def test_sort_full_buckets_equals_library_sort_and_counts_its_phases(pb):
+    """oracle.sort_full_buckets (PAPER.md 3.2, App. B): the result is the sorted input (numpy's sort, an
+    independent routine) for distinct keys, heavy duplicates, 0-1 data, ragged n and every P; the number of
+    rounds of both merge phases is the paper's: ceil(log2(tiles / P)) before the distribution ("suspend the
+    merge at s = P", L131) and ceil(log2 s) = log P inside the buckets (L143)."""
+    rng = np.random.default_rng(31 + pb)
+    w, M = 4, 16                                        # small tiles keep the ShearSort cheap; w = 32 below
+    for trial in range(60):
+        P = int(rng.choice([2, 3, 4, 8]))
+        tiles = int(rng.integers(1, 40))
+        n = tiles * M - int(rng.integers(0, M))
+        kind = trial % 3
+        if kind == 0:
+            keys = rng.permutation(1 << 14)[:n].astype(np.uint32)
+        elif kind == 1:
+            keys = rng.integers(0, 5, size=n).astype(np.uint32)
+        else:
+            keys = rng.integers(0, 2, size=n).astype(np.uint32)
+        t = int(rng.choice([1, 2, P, 2 * P]))
+        runs0 = -(-n // M)
+        r1 = 0
+        while -(-runs0 // (1 << r1)) > P:
+            r1 += 1
+        s = -(-n // (M << r1))
+        if s > 1 and s * t < P:
+            t = P
+        out, info = oracle.sort_full_buckets(keys, P, t=t, pivot_buckets=pb, w=w, return_info=True)
+        assert np.array_equal(out, np.sort(keys, kind="stable"))
+        assert info["first_phase_rounds"] == r1 and info["s"] == s and info["run_len"] == M << r1
+        if s > 1:
+            # log P rounds wherever a bucket is non-empty; only all-pivot data (pivot buckets) has none to merge
+            assert info["final_phase_rounds"] in ((0, _ceil_log2(s)) if pb else (_ceil_log2(s),))
+            assert sum(info["bucket_sizes"]) == n and len(info["bucket_sizes"]) == (2 * P - 1 if pb else P)
+    keys = np.random.default_rng(5).integers(0, 1 << 32, size=20 * 1024 + 77, dtype=np.uint64).astype(np.uint32)
+    assert np.array_equal(oracle.sort_full_buckets(keys, 8, pivot_buckets=pb), np.sort(keys))
+    assert np.array_equal(oracle.sort_full_buckets(keys, 8, pivot_buckets=pb), oracle.sort_full(keys))
+    k64 = np.random.default_rng(6).integers(0, 1 << 63, size=9 * 1024 + 5, dtype=np.uint64)
+    assert np.array_equal(oracle.sort_full_buckets(k64, 4, pivot_buckets=pb), np.sort(k64))
+
+
+def test_sort_full_buckets_pivot_buckets_skip_the_final_phase_on_zero_one_data():
+    """with pivot buckets every key of 0-1 data equals a pivot, so the final merge phase
+    has nothing to merge (0 rounds), while the plain distribution still runs log P rounds in its buckets."""
+    rng = np.random.default_rng(77)
+    keys = rng.integers(0, 2, size=64 * 16).astype(np.uint32)
+    out, info = oracle.sort_full_buckets(keys, 8, pivot_buckets=True, w=4, return_info=True)
+    assert np.array_equal(out, np.sort(keys)) and info["final_phase_rounds"] == 0
+    assert sum(info["bucket_sizes"][0::2]) == 0
+    out, info = oracle.sort_full_buckets(keys, 8, pivot_buckets=False, w=4, return_info=True)
+    assert np.array_equal(out, np.sort(keys)) and info["final_phase_rounds"] == 3
+
+
+def test_merge_round_and_merge_pieces_pins():
+    """oracle.merge_round = one round of oracle.merge_runs (pinned elsewhere against library sorts);
+    oracle.merge_pieces of sorted pieces = the sorted concatenation, ceil(log2 s) rounds, empty pieces allowed."""
+    rng = np.random.default_rng(8)
+    for trial in range(50):
+        n = int(rng.integers(1, 300)); L = int(rng.integers(1, 40))
+        keys = workloads.sorted_runs(rng.integers(0, 9, size=n).astype(np.uint32), L)
+        one = oracle.merge_round(keys, L)
+        assert np.array_equal(one, workloads.sorted_runs(keys, 2 * L))
+        s = int(rng.integers(1, 9))
+        pieces = [np.sort(rng.integers(0, 7, size=int(rng.integers(0, 12))).astype(np.uint32)) for _ in range(s)]
+        merged, rounds = oracle.merge_pieces(pieces)
+        assert np.array_equal(merged, np.sort(np.concatenate(pieces))) and rounds == _ceil_log2(s)
