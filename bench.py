@@ -69,7 +69,8 @@ WORKLOADS = {
     "cfg5b64": ("merge-only, 64 sorted uint32 runs totalling 2^27 keys (config 5)", 27, None, ("merge", 64), "u32"),
     "cfg5b1024": ("merge-only, 1024 sorted uint32 runs totalling 2^27 keys (config 5)", 27, None, ("merge", 1024), "u32"),
 }
-SIDE_WORKLOADS = ("cfg1", "cfg2", "cfg3", "cfg5a", "cfg5b64")   # short device-timed lines beside the headline
+# short device-timed lines beside the headline: every other BASELINE.json config
+SIDE_WORKLOADS = ("cfg4b", "cfg4c", "cfg4d", "cfg4e", "cfg5a", "cfg3", "cfg1", "cfg2", "cfg5b2", "cfg5b64", "cfg5b1024")
 ORACLE_SAMPLE_LOG2 = 25   # ~6 s of single-thread CPU work
 
 
@@ -114,6 +115,7 @@ class Job:
             self.out_k = torch.empty_like(self.src_k)
         self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
         self.passes = None
+        self.opts = None            # bcf_options of this job (None = library defaults)
 
     def restore(self):
         if self.op in ("sort", "tiles"):
@@ -124,11 +126,11 @@ class Job:
     def run(self):
         b = self.bcf
         if self.op == "sort":
-            b.sort(self.k, self.v, workspace=self.ws)
+            b.sort(self.k, self.v, workspace=self.ws, opts=self.opts)
         elif self.op == "tiles":
             (b.sort_tiles_mergesort if TILE_ALGO == "mergesort" else b.sort_tiles)(self.k, self.v)
         else:
-            b.merge_runs(self.src_k, self.run_len, out_keys=self.out_k, workspace=self.ws)
+            b.merge_runs(self.src_k, self.run_len, out_keys=self.out_k, workspace=self.ws, opts=self.opts)
 
     def result(self):
         return self.out_k if isinstance(self.op, tuple) else self.k
@@ -160,6 +162,18 @@ def recorded_traffic(kernel):
     try:
         with open(path) as f:
             return json.load(f).get(kernel)
+    except Exception:
+        return None
+
+
+def recorded_bank_conflicts():
+    """Shared-memory bank-conflict counters per kernel of the committed ncu capture of THIS build
+    (profiles/bank_conflicts.json, written from the ncu CSV by the command named in profiles/r2_conflicts.md):
+    {kernel: {ld, st, wavefronts_ld, wavefronts_st, excess_per_instruction}}; None when no capture is committed."""
+    path = os.path.join(ROOT, "profiles", "bank_conflicts.json")
+    try:
+        with open(path) as f:
+            return json.load(f)
     except Exception:
         return None
 
@@ -307,22 +321,62 @@ def time_steps(torch, job, steps, stream, barrier):
 
 def side_line(bcf, torch, dev, name, stream, barrier, variant=None):
     """A short device-timed measurement of another BASELINE.json config (3 warm-ups, 5 steps).
-    variant: None, or a dict of library / bench settings for this line only
-    ({"base_case": .., "rounds_per_pass": .., "tile_algo": ..})."""
+    variant: None, or a dict of per-call library options / bench settings for this line only
+    ({"base_case": .., "rounds_per_pass": .., "launch_mode": .., "tile_algo": .., "label": ..})."""
     global TILE_ALGO
-    saved = (bcf.get_base_case(), bcf.get_rounds_per_pass(), TILE_ALGO)
+    saved = TILE_ALGO
     if variant:
-        if "base_case" in variant:
-            bcf.set_base_case(variant["base_case"])
-        if "rounds_per_pass" in variant:
-            bcf.set_rounds_per_pass(variant["rounds_per_pass"])
         TILE_ALGO = variant.get("tile_algo", TILE_ALGO)
     try:
         return _side_line(bcf, torch, dev, name, stream, barrier, variant)
     finally:
-        bcf.set_base_case(saved[0])
-        bcf.set_rounds_per_pass(saved[1])
-        TILE_ALGO = saved[2]
+        TILE_ALGO = saved
+
+
+def sort_buckets_lines(bcf, torch, dev, stream):
+    """BCFMergesort with the paper's bucket distribution end to end (bcf_sort_buckets, t = P = 128 = the paper's p)
+    beside plain bcf_sort on the same 2^27 uint32 keys: uniform keys and keys in {0, 1} (the paper's Fig. 4a case,
+    where BCFMergesortPB "has nothing more to do after rearranging the data").  3 warm-ups, 5 steps."""
+    n = 1 << 27
+    rng = np.random.Generator(np.random.Philox(key=workloads.seed_for(6, 1)))
+    inputs = (("uniform keys", workloads.cfg4_sort_u32("uniform", n=n)),
+              ("keys in {0, 1}", rng.integers(0, 2, size=n, dtype=np.uint32)))
+    peak, _ = measured_peak()
+    lines = []
+    for dname, keys in inputs:
+        src = torch.from_numpy(keys.view(np.int32)).to(dev)
+        d = torch.empty_like(src)
+        ws_sort = torch.empty(bcf.workspace_bytes(bcf.binding.OP_SORT, n), dtype=torch.uint8, device=dev)
+        need = int(bcf.lib().bcf_sort_buckets_workspace_bytes(n, 128, 128, 1, 0))
+        ws_b = torch.empty(need, dtype=torch.uint8, device=dev)
+        for label, fn in (("bcf_sort (exact co-rank partitioning)", lambda: bcf.sort(d, workspace=ws_sort)),
+                          ("bcf_sort_buckets, plain buckets (BCFMergesort)", lambda: bcf.sort_buckets(d, 128, workspace=ws_b)),
+                          ("bcf_sort_buckets, pivot buckets (BCFMergesortPB)",
+                           lambda: bcf.sort_buckets(d, 128, pivot_buckets=True, workspace=ws_b))):
+            for _ in range(3):
+                d.copy_(src)
+                fn()
+            torch.cuda.synchronize()
+            if not bool((d[1:] >= d[:-1]).all().item()) and dname != "uniform keys":
+                raise SystemExit("bench: sort_buckets output not sorted")
+            bcf.launch_counts()
+            ms = []
+            for _ in range(5):
+                d.copy_(src)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fn()
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+            launches = bcf.launch_counts()
+            t = sum(ms) / len(ms)
+            lines.append({"workload": "sort_buckets", "description": "sort of 2^27 uint32 keys, " + dname, "variant": label,
+                          "dtype": "u32", "n": n, "value": n / (t * 1e-3), "unit": UNIT, "ms_per_step": t, "best_ms": min(ms),
+                          "gpu_launches_per_step": int(sum(launches.values())) // 5})
+        del src, d, ws_sort, ws_b
+        torch.cuda.empty_cache()
+    return lines
 
 
 def buckets_line(bcf, torch, dev, stream, pivot_buckets, zero_one=False):
@@ -404,6 +458,9 @@ def _side_line(bcf, torch, dev, name, stream, barrier, variant):
     desc, logn, gen, op, dtype = WORKLOADS[name]
     n = 1 << logn
     job = Job(bcf, torch, dev, name, n)
+    if variant:
+        o = {k: variant[k] for k in ("base_case", "rounds_per_pass", "launch_mode", "merge_impl") if k in variant}
+        job.opts = bcf.options(**o) if o else None
     for _ in range(3):
         job.restore()
         job.run()
@@ -439,8 +496,10 @@ def main():
     ap.add_argument("--base-case", default="auto", choices=["auto", "shearsort", "tilemergesort", "longtiles"],
                     help="base case of bcf_sort: the paper's tile ShearSort, the tile mergesort network, long tiles "
                          "(8 tiles per CTA), or auto = the library default (long tiles for u32 keys, tile mergesort else)")
-    ap.add_argument("--rounds-per-pass", type=int, default=1, choices=[1, 2],
-                    help="merge rounds per pass over global memory (2 = four-run kernel)")
+    ap.add_argument("--rounds-per-pass", type=int, default=0, choices=[0, 1, 2],
+                    help="merge rounds per pass over global memory (2 = four-run kernel, 0 = the library default)")
+    ap.add_argument("--launch-mode", default="auto", choices=["auto", "plain", "pdl"],
+                    help="ordinary or programmatic dependent launches (auto = the library default)")
     ap.add_argument("--tile-algo", default="shearsort", choices=["shearsort", "mergesort"],
                     help="network for the batch tile sort workloads cfg1 / cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -473,15 +532,17 @@ def main():
 
     global TILE_ALGO
     TILE_ALGO = args.tile_algo
-    bcf.set_base_case({"shearsort": bcf.BASE_SHEARSORT, "tilemergesort": bcf.BASE_TILE_MERGESORT,
-                       "longtiles": bcf.BASE_LONG_TILES, "auto": bcf.BASE_AUTO}[args.base_case])
-    bcf.set_rounds_per_pass(args.rounds_per_pass)
+    main_opts = bcf.options(base_case={"shearsort": bcf.BASE_SHEARSORT, "tilemergesort": bcf.BASE_TILE_MERGESORT,
+                                       "longtiles": bcf.BASE_LONG_TILES, "auto": bcf.BASE_AUTO}[args.base_case],
+                            rounds_per_pass=args.rounds_per_pass,
+                            launch_mode={"auto": bcf.LAUNCH_AUTO, "plain": bcf.LAUNCH_PLAIN, "pdl": bcf.LAUNCH_PDL}[args.launch_mode])
 
     desc, logn, gen, op, dtype = WORKLOADS[args.workload]
     n = 1 << (args.log2n or logn)
     eb = elem_bytes(dtype)
     # replicas only: every rank works on its own n elements of the same recipe
     job = Job(bcf, torch, dev, args.workload, n, rank)
+    job.opts = main_opts
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -505,6 +566,9 @@ def main():
     t_wall = time.perf_counter() - t_wall
     clocks = sampler.stop()
     prof = bcf.profile_read()
+    if bcf.profile_dropped():
+        raise SystemExit("bench: the library's event pool overflowed (%d launches not timed): use fewer --steps"
+                         % bcf.profile_dropped())
     bcf.profile_enable(False)
     launches = bcf.launch_counts()
     ms = max_over_ranks(sum(step_ms), world, dev)
@@ -566,7 +630,7 @@ def main():
             barrier()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
-            bcf.sort_host(hk, hv, scratch=scratch)
+            bcf.sort_host(hk, hv, scratch=scratch, opts=main_opts)
             b.record(stream)
             torch.cuda.synchronize()
             if i:
@@ -588,43 +652,58 @@ def main():
         dt = oracle_run(args.workload, keys, vals, run_len)
         cpu = {"value": sn / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "host_cores_total": os.cpu_count(), "sample": sample + ", once"}
+    summary = None
+    kv = None
     if rank == 0 and world == 1 and not args.no_side and args.workload == "cfg4a" and not args.log2n:
         del job
         torch.cuda.empty_cache()
         side = [side_line(bcf, torch, dev, w, stream, barrier) for w in SIDE_WORKLOADS]
         # the same configs with the other networks / pass structures the library offers
-        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
-                              {"base_case": bcf.BASE_SHEARSORT, "label": "base case = the paper's tile ShearSort"}))
-        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
-                              {"base_case": bcf.BASE_TILE_MERGESORT, "label": "base case = tile mergesort (one tile per warp)"}))
-        side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier,
-                              {"rounds_per_pass": 2, "label": "two merge rounds per pass (four-run kernel)"}))
-        side.append(side_line(bcf, torch, dev, "cfg1", stream, barrier,
-                              {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
-        side.append(side_line(bcf, torch, dev, "cfg2", stream, barrier,
-                              {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
+        for v in ({"base_case": bcf.BASE_SHEARSORT, "rounds_per_pass": 1, "label": "base case = the paper's tile ShearSort, one round per pass"},
+                  {"base_case": bcf.BASE_TILE_MERGESORT, "rounds_per_pass": 1, "label": "base case = tile mergesort (one tile per warp), one round per pass"},
+                  {"rounds_per_pass": 1, "label": "one merge round per pass (two-run kernel)"},
+                  {"rounds_per_pass": 2, "label": "two merge rounds per pass (four-run kernel)"},
+                  {"launch_mode": bcf.LAUNCH_PLAIN, "label": "ordinary launches"},
+                  {"launch_mode": bcf.LAUNCH_PDL, "label": "programmatic dependent launches"}):
+            side.append(side_line(bcf, torch, dev, "cfg4a", stream, barrier, v))
+        side.append(side_line(bcf, torch, dev, "cfg1", stream, barrier, {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
+        side.append(side_line(bcf, torch, dev, "cfg2", stream, barrier, {"tile_algo": "mergesort", "label": "bcf_sort_tiles_mergesort"}))
         side.append(buckets_line(bcf, torch, dev, stream, False))
         side.append(buckets_line(bcf, torch, dev, stream, True))
         side.append(buckets_line(bcf, torch, dev, stream, True, zero_one=True))
+        side.extend(sort_buckets_lines(bcf, torch, dev, stream))
         side.extend(colored_scan_lines(bcf, torch, dev, stream))
+        # every BASELINE.json config at a glance: G keys/s and fraction of the measured HBM peak for its pass count
+        summary = {args.workload: [round(value / 1e9, 2), round(roofline.get("whole_step", {}).get("frac_of_measured_peak", 0.0), 3)]}
+        for ln in side:
+            if ln["workload"] in SIDE_WORKLOADS and "variant" not in ln:
+                summary[ln["workload"]] = [round(ln["value"] / 1e9, 2), round(ln["frac_of_measured_hbm_peak_for_pass_count"], 3)]
+        kv5a = next(ln for ln in side if ln["workload"] == "cfg5a" and "variant" not in ln)
+        kv = {"workload": "cfg5a", "dtype": kv5a["dtype"], "n": kv5a["n"], "value": kv5a["value"], "unit": UNIT,
+              "ms_per_step": kv5a["ms_per_step"], "passes": kv5a["passes"],
+              "frac_of_measured_hbm_peak_for_pass_count": kv5a["frac_of_measured_hbm_peak_for_pass_count"]}
 
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": dtype, "data": "synthetic",
+            "summary_gkeys_per_s_and_frac_of_hbm_peak": summary,
             "config": {"workload": args.workload, "description": desc, "n": n, "bytes": eb * n,
                        "passes": passes,
                        "base_case": None if op != "sort" else (args.base_case if args.base_case != "auto" else
                                                                "auto: " + ("longtiles" if dtype == "u32" else "tilemergesort")),
                        "tile_network": args.tile_algo if op == "tiles" else None,
-                       "merge_rounds_per_pass": args.rounds_per_pass, "multi_gpu": "replicas only",
+                       "merge_rounds_per_pass": args.rounds_per_pass or "library default", "launch_mode": args.launch_mode,
+                       "multi_gpu": "replicas only",
+                       "kv": kv,
                        "l2": "input and workspace (%d MiB each) %s the 126 MB L2; the input is restored from a "
                              "pristine copy before every step" % (eb * n >> 20, "exceed" if eb * n > 126e6 else "FIT IN"),
                        "timing": "CUDA events around each library call; restore copy outside the events",
                        "best_step_ms": min(step_ms), "wall_s_timed_region": t_wall},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(sum(launches.values())),
-            "launches_by_kernel": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "launches_by_kernel": launches, "profile_launches_not_timed": bcf.profile_dropped(),
+            "roofline": roofline, "bank_conflicts": recorded_bank_conflicts(), "cpu_baseline": cpu,
             "other_workloads": side,
         }))
     if world > 1:

@@ -22,7 +22,14 @@
  *  - ASYNCHRONY: device entry points only enqueue work on `stream` and return; they never
  *    synchronise.  (bcf_sort_host is the exception, see there.)
  *  - ERRORS: status codes only; no exceptions, no exit().  n == 0 is BCF_OK and a no-op.
- *    A failed launch returns BCF_ERR_CUDA and leaves cudaGetLastError() for the caller.
+ *    Every entry point that touches the device first clears a pending (non-sticky) CUDA error of the
+ *    calling thread, checks every launch it makes, stops at the first failure and returns
+ *    BCF_ERR_CUDA once; the CUDA error code of that failure is kept per thread (bcf_last_cuda_error)
+ *    and is not left pending.  After a failure the contents of the output and workspace are unspecified.
+ *  - STATE: the library keeps no settings.  Everything that selects an algorithm is passed per call in a
+ *    bcf_options (below); two threads, or two calls, with different options do not interact.  The only
+ *    process-wide state is the measurement hooks at the end of this file (not thread-safe, off by
+ *    default) and per-device caches of kernel attributes (thread-safe, keyed by device id).
  *  - DEVICE: compute capability 10.x (B200, sm_100a) is required; anything else returns
  *    BCF_ERR_UNSUPPORTED_DEVICE.  There is no fallback path of any kind.
  *  - LIMIT: n < 2^32 elements.
@@ -121,17 +128,42 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
                                bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
 
 /*
- * Base case bcf_sort uses from now on (process-wide, host only): BCF_BASE_SHEARSORT = the paper's
- * tile ShearSort (bcf_sort_tiles), BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort,
- * BCF_BASE_LONG_TILES = bcf_sort_long_tiles with h = 8 (runs of 8192, three merge rounds fewer),
- * BCF_BASE_AUTO = the fastest measured on B200 per element type (long tiles for u32 keys alone, the tile
- * mergesort otherwise).  The result
- * of bcf_sort is the same for both.  Initial value: BCF_BASE_AUTO, or the integer in the
- * environment variable BCF_BASE_CASE.
+ * bcf_options -- per-call algorithm selection.  Pass NULL for the defaults.  No environment variable and no
+ * process-wide setter exists; the result of every entry point is the same for every option value (the
+ * sorted output is unique), only the kernels and the number of passes over global memory differ.
+ *   struct_size     sizeof(bcf_options) of the caller (bcf_options_init fills it); lets the struct grow.
+ *   base_case       base case of bcf_sort: BCF_BASE_SHEARSORT = the paper's tile ShearSort (bcf_sort_tiles),
+ *                   BCF_BASE_TILE_MERGESORT = bcf_sort_tiles_mergesort, BCF_BASE_LONG_TILES =
+ *                   bcf_sort_long_tiles with h = 8 (runs of 8192, three merge rounds fewer), BCF_BASE_AUTO =
+ *                   the fastest measured on B200 per element type.
+ *   rounds_per_pass merge rounds per read + write of the data: 1 (Lemma 2), 2 (four-run kernel
+ *                   where it applies) or 0 = the library's choice.
+ *   merge_impl      BCF_MERGE_IMPL_AUTO, or BCF_MERGE_IMPL_GENERIC = one warp per page with loads from global
+ *                   memory (merge_kernel) even where the TMA-fed pipeline applies.
+ *   partition_warp_search_max
+ *                   largest number of share boundaries of a round searched with 32 lanes per boundary
+ *                   (latency-bound case); above it one thread per boundary.  < 0 = default (4096).
+ *   launch_mode     BCF_LAUNCH_PLAIN = ordinary stream-ordered launches; BCF_LAUNCH_PDL = programmatic
+ *                   dependent launches (a kernel's CTAs are scheduled while its predecessor drains and wait
+ *                   on griddepcontrol before touching its output); BCF_LAUNCH_AUTO = the library's choice
+ *                   (dependent launches for sorts and merges of fewer than 2^26 elements, where launch
+ *                   latency is a measurable share of the run time).
  */
 typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2, BCF_BASE_AUTO = 3 } bcf_base_case;
-bcf_status bcf_set_base_case(int base);
-int bcf_get_base_case(void);
+typedef enum { BCF_MERGE_IMPL_AUTO = 0, BCF_MERGE_IMPL_GENERIC = 1 } bcf_merge_impl;
+typedef enum { BCF_LAUNCH_AUTO = 0, BCF_LAUNCH_PLAIN = 1, BCF_LAUNCH_PDL = 2 } bcf_launch_mode;
+typedef struct bcf_options {
+    uint32_t struct_size;
+    int32_t base_case;
+    int32_t rounds_per_pass;
+    int32_t merge_impl;
+    int32_t partition_warp_search_max;
+    int32_t launch_mode;
+} bcf_options;
+/* Fill *opt with the defaults (AUTO everywhere).  Returns BCF_ERR_INVALID_ARG for NULL. */
+bcf_status bcf_options_init(bcf_options *opt);
+/* CUDA error code (cudaError_t as int) of the calling thread's most recent BCF_ERR_CUDA; 0 if none. */
+int bcf_last_cuda_error(void);
 
 /*
  * bcf_merge_partition -- split-point search of ONE merge pass (hot-path row a5).
@@ -217,20 +249,11 @@ bcf_status bcf_colored_prefix_sums(const uint32_t *d_values, const uint8_t *d_co
 
 /*
  * Number of passes over global memory (one read + one write of all n elements each) that
- * bcf_merge_runs takes from runs of run_len: a pass does two merge rounds where the four-run
- * kernel applies (run_len = 1024 * 2^k and the element type's stage buffers fit one SM) and one
- * round otherwise.  bcf_sort takes 1 + bcf_merge_pass_count(n, BCF_TILE, ..) passes.  Host only.
+ * bcf_merge_runs(_ex) takes from runs of run_len under `opt` (NULL = defaults): a pass does two merge rounds
+ * where the four-run kernel applies (rounds_per_pass = 2, run_len = 1024 * 2^k and the element type's stage
+ * buffers fit one SM) and one round otherwise.  Host only.
  */
-int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt);
-
-/*
- * Merge rounds per pass over global memory used by bcf_merge_runs / bcf_sort from now on
- * (process-wide, host only): 1 = one round per read + write (Lemma 2), 2 = two rounds per
- * read + write with the four-run kernel where it applies.  The result of every entry point is the
- * same for both settings.  Anything else returns BCF_ERR_INVALID_ARG.
- */
-bcf_status bcf_set_rounds_per_pass(int rounds);
-int bcf_get_rounds_per_pass(void);
+int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt, const bcf_options *opt);
 
 /*
  * bcf_merge_runs -- BCFMergesort's merging phase on already sorted runs.
@@ -252,6 +275,10 @@ int bcf_get_rounds_per_pass(void);
 bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
                           size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
                           void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+/* Same with per-call options (NULL = defaults = bcf_merge_runs). */
+bcf_status bcf_merge_runs_ex(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
+                             size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
+                             void *d_workspace, size_t workspace_bytes, bcf_stream_t stream, const bcf_options *opt);
 
 /*
  * bcf_sort -- BCFMergesort (section 3, Appendix B): base case on
@@ -262,6 +289,47 @@ bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_
  */
 bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
                     void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+/* Same with per-call options (NULL = defaults = bcf_sort). */
+bcf_status bcf_sort_ex(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
+                       void *d_workspace, size_t workspace_bytes, bcf_stream_t stream, const bcf_options *opt);
+
+/*
+ * bcf_sort_buckets -- BCFMergesort with the paper's bucket distribution, end to end; with pivot_buckets != 0
+ * this is BCFMergesortPB (section 3.2, section 3.3, Appendix B).  Keys only.
+ * The four phases of the paper in its order:
+ *   1. base case (as bcf_sort);
+ *   2. first merge phase: merge rounds (as bcf_merge_runs) while more than P runs remain -- "we suspend the
+ *      merge at s = P" (L131);
+ *   3. bucket distribution: bcf_find_buckets on the s <= P runs with t samples per run and P buckets
+ *      (2P-1 with pivot buckets);
+ *   4. final merge phase (L141-143): inside every bucket its s sorted pieces (any lengths, possibly empty)
+ *      are merged pairwise in ceil(log2 s) rounds; every round is one launch in which a warp takes one page
+ *      of BCF_TILE outputs of one pair of pieces, finds its split points by co-ranking and merges with
+ *      SHEARSORT-MERGE; partial pages are padded with the maximum key on chip only (L141).  A pivot bucket
+ *      holds copies of one key and is only copied ("already in the correct position", L155).
+ * If one run remains after phase 2 the result is complete and phases 3-4 are skipped.
+ *   d_keys      : n keys, sorted in place.
+ *   P, t        : buckets and samples per run; 2 <= P <= 65536, 1 <= t <= 65536 (the paper: t = P = 128).
+ *   d_workspace : >= bcf_sort_buckets_workspace_bytes(n, t, P, pivot_buckets, kt) bytes.
+ *   d_bucket_starts : NULL, or nb + 1 uint32 (device): start of every bucket in the sorted output, last = n
+ *                 (nb = P or 2P-1); written only when phases 3-4 ran (n > P runs of one tile, more than one run).
+ */
+size_t bcf_sort_buckets_workspace_bytes(size_t n, int t, int P, int pivot_buckets, bcf_key_t kt);
+bcf_status bcf_sort_buckets(void *d_keys, size_t n, bcf_key_t kt, int t, int P, int pivot_buckets,
+                            uint32_t *d_bucket_starts, void *d_workspace, size_t workspace_bytes,
+                            bcf_stream_t stream, const bcf_options *opt);
+
+/*
+ * bcf_merge_pieces -- phase 4 alone: `groups` groups of `s` adjacent sorted pieces each
+ * (piece (g, r) = elements [d_piece_offsets[g s + r], d_piece_offsets[g s + r + 1]) of d_keys_in, the layout
+ * bcf_find_buckets writes) are merged group by group into d_keys_out at the same positions.
+ * copy_odd_groups != 0: groups of odd index are copied instead of merged (pivot buckets).
+ *   d_workspace : >= bcf_merge_pieces_workspace_bytes(n, groups, s, kt) bytes; d_keys_in is not modified.
+ */
+size_t bcf_merge_pieces_workspace_bytes(size_t n, size_t groups, size_t s, bcf_key_t kt);
+bcf_status bcf_merge_pieces(const void *d_keys_in, void *d_keys_out, size_t n, const uint32_t *d_piece_offsets,
+                            size_t groups, size_t s, int copy_odd_groups, bcf_key_t kt, void *d_workspace,
+                            size_t workspace_bytes, bcf_stream_t stream);
 
 /*
  * bcf_sort_host -- bcf_sort on HOST buffers (the end-to-end path bench.py's `e2e` times).
@@ -272,6 +340,8 @@ bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_
  */
 bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
                          void *d_scratch, size_t scratch_bytes, bcf_stream_t stream);
+bcf_status bcf_sort_host_ex(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt,
+                            void *d_scratch, size_t scratch_bytes, bcf_stream_t stream, const bcf_options *opt);
 
 /*
  * bcf_merge_runs_pagewise -- the paper's own streaming form of the merge (hot-path row a7):
@@ -293,8 +363,7 @@ typedef enum {
     BCF_KERNEL_PARTITION = 1,
     BCF_KERNEL_MERGE = 2,
     BCF_KERNEL_MERGE_PAGEWISE = 3,
-    BCF_KERNEL_CLASSES = 4,          /* classes with timing / launch counters                           */
-    BCF_KERNEL_TILE_MERGESORT = 4    /* bcf_kernel_info only; timed and counted as BCF_KERNEL_TILE_SORT */
+    BCF_KERNEL_CLASSES = 4           /* classes with timing / launch counters                           */
 } bcf_kernel_class;
 
 /*
@@ -312,12 +381,37 @@ bcf_status bcf_profile_enable(int on);
 bcf_status bcf_profile_read(float *ms, unsigned long long *launches);
 void bcf_launch_counts(unsigned long long *launches);
 
+/* Launches bcf_profile_enable(1) could not time because its fixed pool of events was full (then
+ * bcf_profile_read's sums are incomplete and say so here); reset by bcf_profile_enable. */
+unsigned long long bcf_profile_dropped(void);
+
 /*
- * Static resource usage of a kernel class for an element type (needs a device):
+ * Static resource usage of every kernel the library can launch, for an element type (needs a device):
  * registers per thread, static+dynamic shared memory per CTA as launched, threads per CTA,
- * resident CTAs per SM at that configuration, local-memory bytes per thread (must be 0).
+ * resident CTAs per SM at that configuration, local-memory bytes per thread.  PAPER.md:L151 makes "the
+ * data is not transferred to local memory" part of the method: tests assert 0 bytes for every kernel.
+ * BCF_ERR_INVALID_ARG for a kernel that does not exist for the element type (merge4_pipe for (u64,u32),
+ * merge_pieces for key-value types).
  */
-bcf_status bcf_kernel_info(int kernel_class, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread,
+typedef enum {
+    BCF_KID_TILE_SORT = 0,
+    BCF_KID_TILE_MERGESORT = 1,
+    BCF_KID_LONG_TILE_2 = 2,
+    BCF_KID_LONG_TILE_4 = 3,
+    BCF_KID_LONG_TILE_8 = 4,
+    BCF_KID_PARTITION = 5,
+    BCF_KID_MERGE = 6,
+    BCF_KID_PARTITION_SHARE_1 = 7,
+    BCF_KID_PARTITION_SHARE_32 = 8,
+    BCF_KID_MERGE_PIPE = 9,
+    BCF_KID_PARTITION4 = 10,
+    BCF_KID_MERGE4_PIPE = 11,
+    BCF_KID_MERGE_PAGEWISE = 12,
+    BCF_KID_MERGE_PIECES = 13,
+    BCF_KID_COUNT = 14
+} bcf_kernel_id;
+const char *bcf_kernel_name(int kernel_id);
+bcf_status bcf_kernel_info(int kernel_id, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread,
                            int *smem_bytes_per_cta, int *threads_per_cta, int *ctas_per_sm,
                            int *local_bytes_per_thread);
 

@@ -10,6 +10,7 @@ missing or the device is not a B200, calls raise.
     out = bcf.merge_runs(keys, run_len)       # sorted runs -> one sequence  (bcf_merge_runs)
     bcf.sort(keys, vals)                      # in place BCFMergesort        (bcf_sort)
 """
+from . import binding  # noqa: F401
 from .binding import (  # noqa: F401
     BcfError,
     KERNEL_CLASSES,
@@ -25,8 +26,19 @@ from .binding import (  # noqa: F401
     merge_partition,
     merge_partition4,
     merge_pass_count,
-    get_rounds_per_pass,
-    set_rounds_per_pass,
+    merge_pieces,
+    sort_buckets,
+    options,
+    Options,
+    KERNEL_IDS,
+    kernel_name,
+    last_cuda_error,
+    profile_dropped,
+    MERGE_IMPL_AUTO,
+    MERGE_IMPL_GENERIC,
+    LAUNCH_AUTO,
+    LAUNCH_PLAIN,
+    LAUNCH_PDL,
     merge_runs,
     merge_runs_pagewise,
     num_shares,
@@ -36,8 +48,6 @@ from .binding import (  # noqa: F401
     sort_host,
     sort_tiles,
     sort_tiles_mergesort,
-    set_base_case,
-    get_base_case,
     BASE_SHEARSORT,
     BASE_TILE_MERGESORT,
     BASE_LONG_TILES,

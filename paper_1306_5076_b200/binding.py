@@ -12,6 +12,46 @@ BCF_KEY_U32, BCF_KEY_U64 = 0, 1
 BCF_VAL_NONE, BCF_VAL_U32 = 0, 1
 OP_SORT_TILES, OP_MERGE_RUNS, OP_SORT, OP_SORT_HOST, OP_MERGE_PAGEWISE = range(5)
 KERNEL_CLASSES = ("tile_sort", "partition", "merge", "merge_pagewise")
+# bcf_kernel_id (include/bcf.h): every kernel the library can launch
+KERNEL_IDS = ("tile_sort", "tile_mergesort", "long_tile_2", "long_tile_4", "long_tile_8", "partition", "merge",
+              "partition_share_1", "partition_share_32", "merge_pipe", "partition4", "merge4_pipe", "merge_pagewise",
+              "merge_pieces")
+BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES, BASE_AUTO = 0, 1, 2, 3
+MERGE_IMPL_AUTO, MERGE_IMPL_GENERIC = 0, 1
+LAUNCH_AUTO, LAUNCH_PLAIN, LAUNCH_PDL = 0, 1, 2
+
+
+class Options(ctypes.Structure):
+    """struct bcf_options (include/bcf.h): per-call algorithm selection; the library keeps no settings."""
+    _fields_ = [("struct_size", ctypes.c_uint32), ("base_case", ctypes.c_int32), ("rounds_per_pass", ctypes.c_int32),
+                ("merge_impl", ctypes.c_int32), ("partition_warp_search_max", ctypes.c_int32),
+                ("launch_mode", ctypes.c_int32)]
+
+
+def options(base_case=None, rounds_per_pass=None, merge_impl=None, partition_warp_search_max=None, launch_mode=None):
+    """A bcf_options filled by bcf_options_init with the given fields overridden (None = the library default)."""
+    o = Options()
+    _check(lib().bcf_options_init(ctypes.byref(o)), "bcf_options_init")
+    if base_case is not None:
+        o.base_case = int(base_case)
+    if rounds_per_pass is not None:
+        o.rounds_per_pass = int(rounds_per_pass)
+    if merge_impl is not None:
+        o.merge_impl = int(merge_impl)
+    if partition_warp_search_max is not None:
+        o.partition_warp_search_max = int(partition_warp_search_max)
+    if launch_mode is not None:
+        o.launch_mode = int(launch_mode)
+    return o
+
+
+def _opt(opts):
+    """None, an Options, or a dict of options() keywords -> pointer argument."""
+    if opts is None:
+        return None
+    if isinstance(opts, dict):
+        opts = options(**opts)
+    return ctypes.byref(opts)
 TILE = 1024
 SHARE = 8192
 
@@ -41,22 +81,34 @@ def lib():
     L.bcf_workspace_bytes.argtypes = [ci, sz, sz, ci, ci]
     L.bcf_sort_tiles.argtypes = [vp, vp, sz, ci, ci, vp]
     L.bcf_sort_tiles_mergesort.argtypes = [vp, vp, sz, ci, ci, vp]
-    L.bcf_set_base_case.argtypes = [ci]
+    L.bcf_options_init.argtypes = [ctypes.POINTER(Options)]
+    L.bcf_last_cuda_error.restype = ci
+    L.bcf_profile_dropped.restype = u64
+    L.bcf_kernel_name.restype = ctypes.c_char_p
+    L.bcf_kernel_name.argtypes = [ci]
     L.bcf_sort_long_tiles.argtypes = [vp, vp, sz, ci, ci, ci, vp]
     L.bcf_merge_partition.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_partition4.argtypes = [vp, vp, sz, sz, ci, ci, vp, sz, vp]
-    L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci]
+    L.bcf_merge_pass_count.argtypes = [sz, sz, ci, ci, vp]
     L.bcf_colored_prefix_sums_workspace_bytes.restype = sz
     L.bcf_colored_prefix_sums_workspace_bytes.argtypes = [sz]
     L.bcf_colored_prefix_sums.argtypes = [vp, vp, sz, ci, ci, vp, vp, sz, vp]
     L.bcf_find_buckets_workspace_bytes.restype = sz
     L.bcf_find_buckets_workspace_bytes.argtypes = [sz, sz, ci, ci, ci, ci]
     L.bcf_find_buckets.argtypes = [vp, sz, sz, ci, ci, ci, ci, vp, vp, vp, vp, sz, vp]
-    L.bcf_set_rounds_per_pass.argtypes = [ci]
     L.bcf_merge_runs.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_runs_pagewise.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_merge_runs_ex.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp, vp]
     L.bcf_sort.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
+    L.bcf_sort_ex.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp, vp]
     L.bcf_sort_host.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
+    L.bcf_sort_host_ex.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp, vp]
+    L.bcf_sort_buckets_workspace_bytes.restype = sz
+    L.bcf_sort_buckets_workspace_bytes.argtypes = [sz, ci, ci, ci, ci]
+    L.bcf_sort_buckets.argtypes = [vp, sz, ci, ci, ci, ci, vp, vp, sz, vp, vp]
+    L.bcf_merge_pieces_workspace_bytes.restype = sz
+    L.bcf_merge_pieces_workspace_bytes.argtypes = [sz, sz, sz, ci]
+    L.bcf_merge_pieces.argtypes = [vp, vp, sz, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_profile_enable.argtypes = [ci]
     L.bcf_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u64)]
     L.bcf_launch_counts.argtypes = [ctypes.POINTER(u64)]
@@ -171,18 +223,6 @@ def sort_long_tiles(keys, h, vals=None, stream=None):
     return keys if vals is None else (keys, vals)
 
 
-BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES, BASE_AUTO = 0, 1, 2, 3
-
-
-def set_base_case(base):
-    """bcf_set_base_case: base case of sort(): BASE_SHEARSORT or BASE_TILE_MERGESORT."""
-    _check(lib().bcf_set_base_case(int(base)), "bcf_set_base_case")
-
-
-def get_base_case():
-    return int(lib().bcf_get_base_case())
-
-
 def merge_partition(keys, run_len, vals=None, stream=None):
     """bcf_merge_partition: split points (uint32 tensor) of one merge round."""
     torch = _torch()
@@ -207,12 +247,12 @@ def merge_partition4(keys, run_len, vals=None, stream=None):
     return splits
 
 
-def merge_pass_count(n, run_len, key_dtype=None, has_vals=False, kt=None, vt=None):
-    """bcf_merge_pass_count: passes over global memory bcf_merge_runs takes from runs of run_len."""
+def merge_pass_count(n, run_len, key_dtype=None, has_vals=False, kt=None, vt=None, opts=None):
+    """bcf_merge_pass_count: passes over global memory bcf_merge_runs takes from runs of run_len under opts."""
     if kt is None:
         kt = BCF_KEY_U64 if np.dtype(key_dtype).itemsize == 8 else BCF_KEY_U32
         vt = BCF_VAL_U32 if has_vals else BCF_VAL_NONE
-    return int(lib().bcf_merge_pass_count(int(n), int(run_len), kt, vt))
+    return int(lib().bcf_merge_pass_count(int(n), int(run_len), kt, vt, _opt(opts)))
 
 
 def find_buckets(keys, run_len, t, P, pivot_buckets=False, stream=None):
@@ -257,16 +297,7 @@ def colored_prefix_sums(values, colors, num_colors, layout=SCAN_BANK_PER_THREAD,
     return out
 
 
-def set_rounds_per_pass(rounds):
-    """bcf_set_rounds_per_pass: 1 or 2 merge rounds per pass over global memory."""
-    _check(lib().bcf_set_rounds_per_pass(int(rounds)), "bcf_set_rounds_per_pass")
-
-
-def get_rounds_per_pass():
-    return int(lib().bcf_get_rounds_per_pass())
-
-
-def _merge(fn, name, op, keys, run_len, vals, out_keys, out_vals, workspace, stream):
+def _merge(fn, name, op, keys, run_len, vals, out_keys, out_vals, workspace, stream, opts=False):
     torch = _torch()
     kt, vt = _types(keys, vals)
     n = keys.numel()
@@ -275,15 +306,16 @@ def _merge(fn, name, op, keys, run_len, vals, out_keys, out_vals, workspace, str
     if vals is not None and out_vals is None:
         out_vals = torch.empty_like(vals)
     ws, ws_bytes = _workspace(op, n, run_len, kt, vt, keys.device, workspace)
-    _check(fn(_dev(keys, "keys"), _dev(vals, "vals"), _dev(out_keys, "out_keys"), _dev(out_vals, "out_vals"),
-              n, int(run_len), kt, vt, ws.data_ptr(), ws_bytes, _stream(stream)), name)
+    args = (_dev(keys, "keys"), _dev(vals, "vals"), _dev(out_keys, "out_keys"), _dev(out_vals, "out_vals"),
+            n, int(run_len), kt, vt, ws.data_ptr(), ws_bytes, _stream(stream))
+    _check(fn(*args) if opts is False else fn(*args, _opt(opts)), name)
     return out_keys if vals is None else (out_keys, out_vals)
 
 
-def merge_runs(keys, run_len, vals=None, out_keys=None, out_vals=None, workspace=None, stream=None):
-    """bcf_merge_runs: merge sorted runs of run_len into one sorted sequence (out of place)."""
-    return _merge(lib().bcf_merge_runs, "bcf_merge_runs", OP_MERGE_RUNS, keys, run_len, vals, out_keys, out_vals,
-                  workspace, stream)
+def merge_runs(keys, run_len, vals=None, out_keys=None, out_vals=None, workspace=None, stream=None, opts=None):
+    """bcf_merge_runs(_ex): merge sorted runs of run_len into one sorted sequence (out of place)."""
+    return _merge(lib().bcf_merge_runs_ex, "bcf_merge_runs_ex", OP_MERGE_RUNS, keys, run_len, vals, out_keys, out_vals,
+                  workspace, stream, opts)
 
 
 def merge_runs_pagewise(keys, run_len, vals=None, out_keys=None, out_vals=None, workspace=None, stream=None):
@@ -292,17 +324,52 @@ def merge_runs_pagewise(keys, run_len, vals=None, out_keys=None, out_vals=None, 
                   out_keys, out_vals, workspace, stream)
 
 
-def sort(keys, vals=None, workspace=None, stream=None):
-    """bcf_sort: in place BCFMergesort of device tensors."""
+def sort(keys, vals=None, workspace=None, stream=None, opts=None):
+    """bcf_sort(_ex): in place BCFMergesort of device tensors.  opts: None, options(...) or a dict of its keywords."""
     kt, vt = _types(keys, vals)
     n = keys.numel()
     ws, ws_bytes = _workspace(OP_SORT, n, 0, kt, vt, keys.device, workspace)
-    _check(lib().bcf_sort(_dev(keys, "keys"), _dev(vals, "vals"), n, kt, vt, ws.data_ptr(), ws_bytes,
-                          _stream(stream)), "bcf_sort")
+    _check(lib().bcf_sort_ex(_dev(keys, "keys"), _dev(vals, "vals"), n, kt, vt, ws.data_ptr(), ws_bytes,
+                             _stream(stream), _opt(opts)), "bcf_sort_ex")
     return keys if vals is None else (keys, vals)
 
 
-def sort_host(keys, vals=None, scratch=None, device="cuda", stream=None):
+def sort_buckets(keys, P, t=None, pivot_buckets=False, workspace=None, stream=None, opts=None, return_bucket_starts=False):
+    """bcf_sort_buckets: BCFMergesort with the paper's bucket distribution (BCFMergesortPB with pivot_buckets),
+    keys only, in place.  With return_bucket_starts also the nb + 1 bucket starts (int32 tensor; only meaningful
+    when the distribution ran, i.e. more than one run was left after the first merge phase)."""
+    torch = _torch()
+    kt, _ = _types(keys, None)
+    n = keys.numel()
+    t = P if t is None else t
+    need = int(lib().bcf_sort_buckets_workspace_bytes(n, int(t), int(P), int(bool(pivot_buckets)), kt))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=keys.device)
+    nb = 2 * P - 1 if pivot_buckets else P
+    starts = torch.full((nb + 1,), -1, dtype=torch.int32, device=keys.device) if return_bucket_starts else None
+    _check(lib().bcf_sort_buckets(_dev(keys, "keys"), n, kt, int(t), int(P), int(bool(pivot_buckets)),
+                                  None if starts is None else starts.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                  _stream(stream), _opt(opts)), "bcf_sort_buckets")
+    return (keys, starts) if return_bucket_starts else keys
+
+
+def merge_pieces(keys, piece_offsets, groups, s, copy_odd_groups=False, out_keys=None, workspace=None, stream=None):
+    """bcf_merge_pieces: the final merge phase alone on the layout bcf_find_buckets writes."""
+    torch = _torch()
+    kt, _ = _types(keys, None)
+    n = keys.numel()
+    if out_keys is None:
+        out_keys = torch.empty_like(keys)
+    need = int(lib().bcf_merge_pieces_workspace_bytes(n, int(groups), int(s), kt))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=keys.device)
+    _check(lib().bcf_merge_pieces(_dev(keys, "keys"), _dev(out_keys, "out_keys"), n, _dev(piece_offsets, "piece_offsets"),
+                                  int(groups), int(s), int(bool(copy_odd_groups)), kt, workspace.data_ptr(),
+                                  workspace.numel(), _stream(stream)), "bcf_merge_pieces")
+    return out_keys
+
+
+def sort_host(keys, vals=None, scratch=None, device="cuda", stream=None, opts=None):
     """bcf_sort_host: in place sort of HOST tensors (ideally pinned); H2D + sort + D2H + sync."""
     torch = _torch()
     kt, vt = _types(keys, vals)
@@ -312,8 +379,8 @@ def sort_host(keys, vals=None, scratch=None, device="cuda", stream=None):
     need = int(lib().bcf_workspace_bytes(OP_SORT_HOST, n, 0, kt, vt))
     if scratch is None:
         scratch = torch.empty(max(need, 16), dtype=torch.uint8, device=device)
-    _check(lib().bcf_sort_host(keys.data_ptr(), None if vals is None else vals.data_ptr(), n, kt, vt,
-                               scratch.data_ptr(), scratch.numel(), _stream(stream)), "bcf_sort_host")
+    _check(lib().bcf_sort_host_ex(keys.data_ptr(), None if vals is None else vals.data_ptr(), n, kt, vt,
+                                  scratch.data_ptr(), scratch.numel(), _stream(stream), _opt(opts)), "bcf_sort_host_ex")
     return keys if vals is None else (keys, vals)
 
 
@@ -335,10 +402,26 @@ def launch_counts():
     return {k: int(cnt[i]) for i, k in enumerate(KERNEL_CLASSES)}
 
 
-def kernel_info(kernel_class, kt=BCF_KEY_U32, vt=BCF_VAL_NONE):
+def profile_dropped():
+    """Launches the profiler could not time because its event pool was full (bcf_profile_dropped)."""
+    return int(lib().bcf_profile_dropped())
+
+
+def last_cuda_error():
+    return int(lib().bcf_last_cuda_error())
+
+
+def kernel_name(kernel_id):
+    cid = kernel_id if isinstance(kernel_id, int) else KERNEL_IDS.index(kernel_id)
+    name = lib().bcf_kernel_name(cid)
+    return None if name is None else name.decode()
+
+
+def kernel_info(kernel_id, kt=BCF_KEY_U32, vt=BCF_VAL_NONE):
+    """bcf_kernel_info of a kernel named in KERNEL_IDS (or its integer id)."""
     vals = [ctypes.c_int() for _ in range(5)]
-    cls = kernel_class if isinstance(kernel_class, int) else KERNEL_CLASSES.index(kernel_class)
-    _check(lib().bcf_kernel_info(cls, kt, vt, *[ctypes.byref(v) for v in vals]),
+    cid = kernel_id if isinstance(kernel_id, int) else KERNEL_IDS.index(kernel_id)
+    _check(lib().bcf_kernel_info(cid, kt, vt, *[ctypes.byref(v) for v in vals]),
            "bcf_kernel_info")
     names = ("regs_per_thread", "smem_bytes_per_cta", "threads_per_cta", "ctas_per_sm", "local_bytes_per_thread")
     return dict(zip(names, (v.value for v in vals)))

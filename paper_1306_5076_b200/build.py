@@ -1,39 +1,76 @@
 """Build libbcf.so (the C-ABI CUDA library, include/bcf.h) in-tree with nvcc for sm_100a.
 
-Usage: python -m paper_1306_5076_b200.build [--force]      (also called by __graft_entry__.build()).
-nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with gpurun.
+Usage: python -m paper_1306_5076_b200.build [--force] [-v]      (also called by __graft_entry__.build()).
+nvcc cross-compiles without a GPU.  The library is several translation units (csrc/bcf_api.cu = the C ABI and
+the driver, csrc/bcf_tu_*.cu = one kernel family each) compiled in parallel into build/*.o and linked into
+libbcf.so; a unit is recompiled when its source, a header under csrc/ or include/bcf.h is newer than its
+object.  Objects and the .so are git-ignored; the .so travels to the GPU box with gpurun.
 """
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libbcf.so")
-SOURCES = ["bcf_api.cu"]
+SOURCES = ["bcf_api.cu", "bcf_tu_tile.cu", "bcf_tu_long.cu", "bcf_tu_merge.cu", "bcf_tu_pipe.cu", "bcf_tu_merge4.cu",
+           "bcf_tu_buckets.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-Xcompiler", "-fPIC",
 ]
 
 
-def _newest_source_mtime():
+def _headers_mtime():
     newest = os.path.getmtime(os.path.join(HERE, "..", "include", "bcf.h"))
     for f in os.listdir(CSRC):
-        newest = max(newest, os.path.getmtime(os.path.join(CSRC, f)))
+        if f.endswith((".cuh", ".h")):
+            newest = max(newest, os.path.getmtime(os.path.join(CSRC, f)))
     return newest
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(OUT) and os.path.getmtime(OUT) >= _newest_source_mtime():
-        return OUT
+def _compile(nvcc, src, obj, verbose, extra):
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+    r = subprocess.run(cmd, cwd=HERE, capture_output=True, text=True)
+    return src, r.returncode, r.stdout + r.stderr
+
+
+def build(force: bool = False, verbose: bool = False, extra_flags=(), log=None) -> str:
+    """Compile what is out of date and link.  `extra_flags` (e.g. -D...) are for A/B experiments only; they force
+    a full rebuild.  `log`: file that receives the compiler output (ptxas -v lines with verbose)."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", OUT] + \
-        [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.check_call(cmd, cwd=HERE)
+    os.makedirs(OBJ, exist_ok=True)
+    hdr = _headers_mtime()
+    force = force or bool(extra_flags)
+    todo = []
+    for s in SOURCES:
+        src = os.path.join(CSRC, s)
+        obj = os.path.join(OBJ, s[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr, os.path.getmtime(src)):
+            todo.append((src, obj))
+    objs = [os.path.join(OBJ, s[:-3] + ".o") for s in SOURCES]
+    if not todo and os.path.exists(OUT) and os.path.getmtime(OUT) >= max(os.path.getmtime(o) for o in objs):
+        return OUT
+    outputs = []
+    with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 1) or 1) as ex:
+        for src, rc, out in ex.map(lambda so: _compile(nvcc, so[0], so[1], verbose, list(extra_flags)), todo):
+            outputs.append("==== %s (rc %d)\n%s" % (os.path.basename(src), rc, out))
+            if rc != 0:
+                if log:
+                    with open(log, "w") as f:
+                        f.write("\n".join(outputs))
+                raise RuntimeError("nvcc failed on %s:\n%s" % (src, out[-4000:]))
+    if log:
+        with open(log, "w") as f:
+            f.write("\n".join(outputs))
+    subprocess.check_call([nvcc, "-shared", "-o", OUT] + objs, cwd=HERE)
     return OUT
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    flags = [a for a in sys.argv[1:] if a.startswith("-D")]
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, extra_flags=flags,
+                log=os.environ.get("BCF_BUILD_LOG")))

@@ -1,46 +1,25 @@
 // bcf_api.cu -- the C ABI of include/bcf.h: argument validation, workspace carving, the merge-round
 // driver and the measurement hooks.  Every step of the path runs in the
-// kernels of bcf_kernels.cuh; there is no CPU fallback.
-#include "../../include/bcf.h"
+// kernels (one translation unit per kernel family, bcf_tu_*.cu); there is no CPU fallback.
+#include "bcf_internal.cuh"
 
 #include <cstdio>
 #include <cstring>
-
-#include "bcf_kernels.cuh"
-#include "bcf_pagewise.cuh"
-#include "bcf_merge_pipe.cuh"
-#include "bcf_merge4.cuh"
-#include "bcf_long_tile.cuh"
-#include "bcf_buckets.cuh"
-#include "bcf_colored_scan.cuh"
-#include <cstdlib>
+#include <initializer_list>
 
 using namespace bcf;
 
+namespace bcf {
+
+int &last_cuda_error_ref()
+{
+    thread_local int e = 0;
+    return e;
+}
+
+}  // namespace bcf
+
 namespace {
-
-// ------------------------------------------------------------------ small host helpers
-
-inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-inline int ceil_log2(size_t x) { int l = 0; while ((size_t(1) << l) < x) ++l; return l; }
-inline size_t key_bytes(bcf_key_t kt) { return kt == BCF_KEY_U64 ? 8 : 4; }
-inline bool valid_types(bcf_key_t kt, bcf_val_t vt)
-{
-    return (kt == BCF_KEY_U32 || kt == BCF_KEY_U64) && (vt == BCF_VAL_NONE || vt == BCF_VAL_U32);
-}
-
-PassGeom pass_geom(size_t n, size_t run_len)
-{
-    PassGeom g;
-    g.n = n;
-    g.run_len = run_len;
-    const unsigned long long two_l = 2ull * run_len;
-    g.shares_per_pair = static_cast<unsigned int>((two_l + TILE - 1) / TILE);
-    const unsigned long long pairs = (n + two_l - 1) / two_l;
-    g.num_shares = pairs * g.shares_per_pair;
-    return g;
-}
 
 // Largest split-point array any round of merging runs of `run_len` needs.
 size_t max_shares(size_t n, size_t run_len)
@@ -53,18 +32,71 @@ size_t max_shares(size_t n, size_t run_len)
     return m;
 }
 
-bcf_status check_device()
+// ------------------------------------------------------------------ per-device state (keyed by device id)
+
+struct DevCache {
+    std::atomic<int> state{0};   // 0 unknown, 1 supported, 2 unsupported
+    int num_sms = 0;
+};
+DevCache g_dev[MAX_DEVICES];
+
+// The current device: clears a stale pending error, checks compute capability 10.x once per device.
+bcf_status current_device(Dev *d)
 {
-    static int cached_dev = -1;
-    static bcf_status cached = BCF_ERR_UNSUPPORTED_DEVICE;
+    (void)cudaGetLastError();
     int dev = -1;
-    if (cudaGetDevice(&dev) != cudaSuccess) return BCF_ERR_CUDA;
-    if (dev == cached_dev) return cached;
-    int major = 0;
-    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return BCF_ERR_CUDA;
-    cached_dev = dev;
-    cached = (major == 10) ? BCF_OK : BCF_ERR_UNSUPPORTED_DEVICE;
-    return cached;
+    BCF_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) return BCF_ERR_UNSUPPORTED_DEVICE;
+    DevCache &c = g_dev[dev];
+    int st = c.state.load(std::memory_order_acquire);
+    if (st == 0) {
+        int major = 0, sms = 0;
+        BCF_CUDA(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        BCF_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        c.num_sms = sms;
+        st = (major == 10) ? 1 : 2;
+        c.state.store(st, std::memory_order_release);
+    }
+    if (st != 1) return BCF_ERR_UNSUPPORTED_DEVICE;
+    d->id = dev;
+    d->num_sms = c.num_sms;
+    return BCF_OK;
+}
+
+// ------------------------------------------------------------------ per-call options (bcf_options)
+
+#ifndef BCF_DEFAULT_ROUNDS_PER_PASS
+#define BCF_DEFAULT_ROUNDS_PER_PASS 1
+#endif
+// BCF_LAUNCH_AUTO: programmatic dependent launches below this many elements.  Measured on B200:
+// they hide the launch latency between the ~2 launches of every merge round, which is 27 % of a 2^20-key sort and
+// 11 % of a 2^24-key sort, but cost 2 % at 2^28 keys where every launch runs for a third of a millisecond.
+#ifndef BCF_PDL_AUTO_MAX_N
+#define BCF_PDL_AUTO_MAX_N (size_t(1) << 26)
+#endif
+
+bool resolve_options(const bcf_options *o, Opt *r)
+{
+    *r = Opt();
+    r->rounds_per_pass = BCF_DEFAULT_ROUNDS_PER_PASS;
+    if (!o) return true;
+    if (o->struct_size < sizeof(bcf_options)) return false;
+    if (o->base_case < BCF_BASE_SHEARSORT || o->base_case > BCF_BASE_AUTO) return false;
+    if (o->rounds_per_pass < 0 || o->rounds_per_pass > 2) return false;
+    if (o->merge_impl != BCF_MERGE_IMPL_AUTO && o->merge_impl != BCF_MERGE_IMPL_GENERIC) return false;
+    if (o->launch_mode < BCF_LAUNCH_AUTO || o->launch_mode > BCF_LAUNCH_PDL) return false;
+    r->base_case = o->base_case;
+    if (o->rounds_per_pass) r->rounds_per_pass = o->rounds_per_pass;
+    r->generic_merge = o->merge_impl == BCF_MERGE_IMPL_GENERIC;
+    if (o->partition_warp_search_max >= 0) r->warp_search_max = static_cast<unsigned long long>(o->partition_warp_search_max);
+    r->launch_mode = o->launch_mode;
+    return true;
+}
+
+// launch mode of a call that works on n elements
+inline void resolve_launch_mode(Opt *o, size_t n)
+{
+    o->pdl = o->launch_mode == BCF_LAUNCH_PDL || (o->launch_mode == BCF_LAUNCH_AUTO && n < BCF_PDL_AUTO_MAX_N);
 }
 
 bool overlap(const void *a, size_t an, const void *b, size_t bn)
@@ -87,12 +119,14 @@ struct Profile {
     int cls[PROFILE_POOL];             // kernel class of the launch that starts at ev[i]; -1: closing event
     int created = 0;
     int open_since = -1;               // first entry of the API call in progress
+    unsigned long long dropped = 0;    // launches not timed because the pool was full
     unsigned long long launches[BCF_KERNEL_CLASSES] = {0, 0, 0, 0};
 } g_prof;
 
 inline int profile_mark(int cls, cudaStream_t s)
 {
-    if (!g_prof.on || g_prof.used >= PROFILE_POOL) return -1;
+    if (!g_prof.on) return -1;
+    if (g_prof.used >= PROFILE_POOL) { g_prof.dropped++; return -1; }
     const int idx = g_prof.used++;
     if (idx >= g_prof.created) {
         cudaEventCreate(&g_prof.ev[idx]);
@@ -103,13 +137,15 @@ inline int profile_mark(int cls, cudaStream_t s)
     return idx;
 }
 
-struct LaunchTimer {
-    LaunchTimer(int cls, cudaStream_t stream)
-    {
-        g_prof.launches[cls]++;
-        profile_mark(cls, stream);
-    }
-};
+}  // namespace
+
+void bcf::profile_launch(int cls, cudaStream_t stream)
+{
+    g_prof.launches[cls]++;
+    profile_mark(cls, stream);
+}
+
+namespace {
 
 // Closes the timed launches of one public API call (outermost scope only).
 struct ProfileGroup {
@@ -127,285 +163,22 @@ struct ProfileGroup {
     }
 };
 
-// ------------------------------------------------------------------ launchers
-
-template <class E>
-constexpr size_t warp_smem_bytes() { return size_t(E::NP) * TILE * 4; }
-
-// Base case of bcf_sort: BCF_BASE_SHEARSORT (the paper's tile sort), BCF_BASE_TILE_MERGESORT (same tile,
-// same movement, mergers instead of full line sorts; bcf_kernels.cuh), BCF_BASE_LONG_TILES (8 tiles per CTA,
-// bcf_long_tile.cuh) or BCF_BASE_AUTO.  bcf_set_base_case().
-#ifndef BCF_DEFAULT_BASE_CASE
-#define BCF_DEFAULT_BASE_CASE BCF_BASE_AUTO
-#endif
-int g_base_case = -1;
-inline int base_case()
-{
-    if (g_base_case < 0) {
-        const char *e = std::getenv("BCF_BASE_CASE");
-        const int v = e ? std::atoi(e) : BCF_DEFAULT_BASE_CASE;
-        g_base_case = (v >= BCF_BASE_SHEARSORT && v <= BCF_BASE_AUTO) ? v : BCF_DEFAULT_BASE_CASE;
-    }
-    return g_base_case;
-}
-
-template <class E>
-bcf_status launch_tile_sort(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n,
-                            cudaStream_t s, int algo = BCF_BASE_SHEARSORT)
-{
-    const size_t tiles = (n + TILE - 1) / TILE;
-    if (tiles == 0) return BCF_OK;
-    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(tile_sort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-            cudaFuncSetAttribute(tile_mergesort_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return BCF_ERR_CUDA;
-        attr_set = true;
-    }
-    const size_t blocks = (tiles + WARPS_PER_CTA - 1) / WARPS_PER_CTA;
-    {
-        LaunchTimer t(BCF_KERNEL_TILE_SORT, s);
-        if (algo == BCF_BASE_TILE_MERGESORT)
-            tile_mergesort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
-        else
-            tile_sort_kernel<E><<<static_cast<unsigned>(blocks), WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
-
-// Long tiles (bcf_long_tile.cuh): groups of h = 2, 4 or 8 tiles sorted by one CTA of h warps.
-#ifndef BCF_LONG_TILE_H
-#define BCF_LONG_TILE_H 8
-#endif
-template <class E, int H>
-bcf_status launch_long_tile_h(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, cudaStream_t s)
-{
-    using C = LongTileCfg<E, H>;
-    static int num_sms = 0, ctas = 0;
-    if (!num_sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            return BCF_ERR_CUDA;
-        if (cudaFuncSetAttribute(long_tile_sort_kernel<E, H>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, long_tile_sort_kernel<E, H>, H * 32, C::smem) != cudaSuccess ||
-            ctas < 1) {
-            num_sms = 0;
-            return BCF_ERR_CUDA;
-        }
-    }
-    const size_t groups = ((n + TILE - 1) / TILE + H - 1) / H;
-    if (groups == 0) return BCF_OK;
-    const size_t cap = static_cast<size_t>(ctas) * num_sms * 8;     // a few waves; the kernel strides over groups
-    {
-        LaunchTimer t(BCF_KERNEL_TILE_SORT, s);
-        long_tile_sort_kernel<E, H><<<static_cast<unsigned>(groups < cap ? groups : cap), H * 32, C::smem, s>>>(kin, vin, kout, vout, n);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
-
-template <class E>
-bcf_status launch_long_tile(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, int h, cudaStream_t s)
-{
-    switch (h) {
-    case 2: return launch_long_tile_h<E, 2>(kin, vin, kout, vout, n, s);
-    case 4: return launch_long_tile_h<E, 4>(kin, vin, kout, vout, n, s);
-    case 8: return launch_long_tile_h<E, 8>(kin, vin, kout, vout, n, s);
-    }
-    return BCF_ERR_INVALID_ARG;
-}
-
-template <class E>
-bcf_status launch_partition(const void *kin, const uint32_t *vin, uint32_t *splits, const PassGeom &g, cudaStream_t s)
-{
-    if (g.num_shares == 0) return BCF_OK;
-    const unsigned blocks = static_cast<unsigned>((g.num_shares + 127) / 128);
-    {
-        LaunchTimer t(BCF_KERNEL_PARTITION, s);
-        partition_kernel<E><<<blocks, 128, 0, s>>>(kin, vin, splits, g);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
-
-template <class E>
-bcf_status launch_merge(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const uint32_t *splits,
-                        const PassGeom &g, cudaStream_t s)
-{
-    if (g.num_shares == 0) return BCF_OK;
-    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(merge_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return BCF_ERR_CUDA;
-        attr_set = true;
-    }
-    const unsigned blocks = static_cast<unsigned>((g.num_shares + WARPS_PER_CTA - 1) / WARPS_PER_CTA);
-    {
-        LaunchTimer t(BCF_KERNEL_MERGE, s);
-        merge_kernel<E><<<blocks, WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, splits, g);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
+// ------------------------------------------------------------------ launch helpers of the driver
 
 // Power-of-two multiples of the tile size take the pipelined kernel (bcf_merge_pipe.cuh).
-inline bool pipe_eligible(size_t run_len)
+inline bool pipe_eligible(size_t run_len, const Opt &o)
 {
     if (run_len % TILE) return false;
     const size_t r = run_len / TILE;
     if (r & (r - 1)) return false;
-    static int forced_v1 = -1;
-    if (forced_v1 < 0) {
-        const char *e = std::getenv("BCF_MERGE_IMPL");
-        forced_v1 = (e && std::strcmp(e, "v1") == 0) ? 1 : 0;
-    }
-    return !forced_v1;
-}
-
-// Largest boundary count that takes the 32-lanes-per-boundary search (BCF_PART_WARP_MAX overrides).
-inline unsigned long long pipe_warp_search_max()
-{
-    static long long v = -1;
-    if (v < 0) {
-        const char *e = std::getenv("BCF_PART_WARP_MAX");
-        v = e ? std::atoll(e) : 4096;
-    }
-    return static_cast<unsigned long long>(v);
-}
-
-template <class E>
-bcf_status launch_merge_pipe(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits, size_t n,
-                             size_t run_len, cudaStream_t s)
-{
-    using C = pipe::Cfg<E>;
-    const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
-    if (shares == 0) return BCF_OK;
-    static int num_sms = 0;
-    if (!num_sms) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-            return BCF_ERR_CUDA;
-        if (cudaFuncSetAttribute(pipe::merge_pipe_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)C::total) != cudaSuccess) {
-            num_sms = 0;
-            return BCF_ERR_CUDA;
-        }
-    }
-    if (2 * run_len > (size_t)pipe::SH) {
-        LaunchTimer t(BCF_KERNEL_PARTITION, s);
-        // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
-        if (shares + 1 <= pipe_warp_search_max()) {
-            const unsigned blocks = static_cast<unsigned>(((shares + 1) * 32 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-            pipe::partition_share_kernel<E, 32><<<blocks, pipe::PART_THREADS, 0, s>>>(kin, vin, splits, n, run_len, shares);
-        } else {
-            const unsigned blocks = static_cast<unsigned>((shares + 1 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-            pipe::partition_share_kernel<E, 1><<<blocks, pipe::PART_THREADS, 0, s>>>(kin, vin, splits, n, run_len, shares);
-        }
-    }
-    {
-        LaunchTimer t(BCF_KERNEL_MERGE, s);
-        const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * num_sms;
-        const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
-        pipe::merge_pipe_kernel<E><<<blocks, pipe::THREADS, C::total, s>>>(kin, vin, kout, vout, splits, n, run_len, shares);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
-
-// Rounds per pass: 2 = the four-run kernel of bcf_merge4.cuh where it applies, 1 = one round per pass
-// everywhere.  Set by bcf_set_rounds_per_pass(); the initial value comes from BCF_MERGE_WAYS (2 or 4 runs
-// per pass) if set.
-#ifndef BCF_DEFAULT_ROUNDS_PER_PASS
-#define BCF_DEFAULT_ROUNDS_PER_PASS 1
-#endif
-int g_rounds_per_pass = -1;
-inline int rounds_per_pass()
-{
-    if (g_rounds_per_pass < 0) {
-        const char *e = std::getenv("BCF_MERGE_WAYS");
-        g_rounds_per_pass = e ? (std::atoi(e) == 4 ? 2 : 1) : BCF_DEFAULT_ROUNDS_PER_PASS;
-    }
-    return g_rounds_per_pass;
+    return !o.generic_merge;
 }
 
 // Element types whose two stage buffers of a four-run share fit one SM (bcf_merge4.cuh).
 template <class E>
-inline bool merge4_eligible(size_t run_len)
+inline bool merge4_eligible(size_t run_len, const Opt &o)
 {
-    return pipe4::Cfg4<E>::fits && pipe_eligible(run_len) && rounds_per_pass() == 2;
-}
-
-template <class E>
-bcf_status launch_partition4(const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len,
-                             size_t num_bounds, cudaStream_t s)
-{
-    if (num_bounds == 0) return BCF_OK;
-    const unsigned blocks = static_cast<unsigned>((num_bounds + pipe4::PART4_THREADS - 1) / pipe4::PART4_THREADS);
-    {
-        LaunchTimer t(BCF_KERNEL_PARTITION, s);
-        pipe4::partition4_kernel<E><<<blocks, pipe4::PART4_THREADS, 0, s>>>(kin, vin, reinterpret_cast<uint4 *>(splits), n, run_len,
-                                                                           num_bounds, pipe4::SH);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-}
-
-// One pass = two merge rounds: groups of four runs of run_len become one run of 4 run_len.
-template <class E>
-bcf_status launch_merge4(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits, size_t n,
-                         size_t run_len, cudaStream_t s)
-{
-    using C = pipe4::Cfg4<E>;
-    if constexpr (!C::fits) {
-        return BCF_ERR_INVALID_ARG;
-    } else {
-        const unsigned long long shares = (n + pipe4::SH - 1) / pipe4::SH;
-        if (shares == 0) return BCF_OK;
-        static int num_sms = 0;
-        if (!num_sms) {
-            int dev = 0;
-            if (cudaGetDevice(&dev) != cudaSuccess ||
-                cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-                return BCF_ERR_CUDA;
-            if (cudaFuncSetAttribute(pipe4::merge4_pipe_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)C::total) != cudaSuccess) {
-                num_sms = 0;
-                return BCF_ERR_CUDA;
-            }
-        }
-        if (4 * run_len > (size_t)pipe4::SH) {
-            const bcf_status st = launch_partition4<E>(kin, vin, splits, n, run_len, shares + 1, s);
-            if (st != BCF_OK) return st;
-        }
-        {
-            LaunchTimer t(BCF_KERNEL_MERGE, s);
-            const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * num_sms;
-            const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
-            pipe4::merge4_pipe_kernel<E><<<blocks, pipe4::THREADS, C::total, s>>>(
-                kin, vin, kout, vout, reinterpret_cast<const uint4 *>(splits), n, run_len, shares);
-        }
-        return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
-    }
-}
-
-template <class E>
-bcf_status launch_pagewise(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, size_t n, size_t run_len,
-                           cudaStream_t s)
-{
-    const size_t pairs = (n + 2 * run_len - 1) / (2 * run_len);
-    if (pairs == 0) return BCF_OK;
-    const size_t smem = WARPS_PER_CTA * warp_smem_bytes<E>();
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(pagewise_merge_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return BCF_ERR_CUDA;
-        attr_set = true;
-    }
-    const unsigned blocks = static_cast<unsigned>((pairs + WARPS_PER_CTA - 1) / WARPS_PER_CTA);
-    {
-        LaunchTimer t(BCF_KERNEL_MERGE_PAGEWISE, s);
-        pagewise_merge_kernel<E><<<blocks, WARPS_PER_CTA * 32, smem, s>>>(kin, vin, kout, vout, n, run_len);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+    return merge4_fits<E>() && pipe_eligible(run_len, o) && o.rounds_per_pass == 2;
 }
 
 // Dispatch a templated callable on the runtime element type.
@@ -440,55 +213,56 @@ Workspace carve(void *base, size_t n, bcf_key_t kt, bcf_val_t vt, bool with_data
     return w;
 }
 
-// The passes of the merging phase from sorted runs of run_len: ways[i] = 2 is one merge
-// round per read + write of the data (Lemma 2), ways[i] = 4 two rounds per read + write
-// (bcf_merge4.cuh).  An odd number of remaining rounds is made even by a two-way pass first.
+// The passes of the merging phase from sorted runs of run_len up to runs of at least
+// `stop_len`: ways[i] = 2 is one merge round per read + write of the data (Lemma 2), ways[i] = 4 two rounds
+// per read + write (bcf_merge4.cuh).  An odd number of remaining rounds is made even by a two-way pass first.
 constexpr int MAX_PASSES = 40;
 template <class E>
-int plan_passes(size_t n, size_t run_len, int *ways)
+int plan_passes(size_t n, size_t run_len, size_t stop_len, const Opt &o, int *ways)
 {
     int np = 0;
-    for (size_t l = run_len; l < n && np < MAX_PASSES; ++np) {
-        const int remaining = ceil_log2((n + l - 1) / l);
-        const bool four = remaining % 2 == 0 && merge4_eligible<E>(l);
+    const size_t target = stop_len < n ? stop_len : n;
+    for (size_t l = run_len; l < target && np < MAX_PASSES; ++np) {
+        const int remaining = ceil_log2((target + l - 1) / l);
+        const bool four = remaining % 2 == 0 && merge4_eligible<E>(l, o);
         ways[np] = four ? 4 : 2;
         l *= four ? 4 : 2;
     }
     return np;
 }
 
-int count_passes(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
+int count_passes(size_t n, size_t run_len, size_t stop_len, bcf_key_t kt, bcf_val_t vt, const Opt &o)
 {
     int ways[MAX_PASSES];
     int np = 0;
-    BCF_DISPATCH(kt, vt, np = plan_passes<E>(n, run_len, ways));
+    BCF_DISPATCH(kt, vt, np = plan_passes<E>(n, run_len, stop_len, o, ways));
     return np;
 }
 
 // Pass i writes to dst[i]; each pass is one read + one write of all n elements.
 template <class E>
-bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
-                        bool first_to_a, size_t n, size_t run_len, uint32_t *splits, cudaStream_t s)
+bcf_status merge_rounds(const Call &c, const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
+                        bool first_to_a, size_t n, size_t run_len, size_t stop_len, uint32_t *splits)
 {
     const void *ksrc = k0;
     const uint32_t *vsrc = v0;
     bool to_a = first_to_a;
     int ways[MAX_PASSES];
-    const int np = plan_passes<E>(n, run_len, ways);
+    const int np = plan_passes<E>(n, run_len, stop_len, c.opt, ways);
     size_t l = run_len;
     for (int i = 0; i < np; ++i) {
         void *kd = to_a ? ka : kb;
         uint32_t *vd = to_a ? va : vb;
         bcf_status st;
         if (ways[i] == 4) {
-            st = launch_merge4<E>(ksrc, vsrc, kd, vd, splits, n, l, s);
-        } else if (pipe_eligible(l)) {
-            st = launch_merge_pipe<E>(ksrc, vsrc, kd, vd, splits, n, l, s);
+            st = launch_merge4<E>(c, ksrc, vsrc, kd, vd, splits, n, l);
+        } else if (pipe_eligible(l, c.opt)) {
+            st = launch_merge_pipe<E>(c, ksrc, vsrc, kd, vd, splits, n, l);
         } else {
             const PassGeom g = pass_geom(n, l);
-            st = launch_partition<E>(ksrc, vsrc, splits, g, s);
+            st = launch_partition<E>(c, ksrc, vsrc, splits, g);
             if (st != BCF_OK) return st;
-            st = launch_merge<E>(ksrc, vsrc, kd, vd, splits, g, s);
+            st = launch_merge<E>(c, ksrc, vsrc, kd, vd, splits, g);
         }
         if (st != BCF_OK) return st;
         ksrc = kd;
@@ -500,8 +274,8 @@ bcf_status merge_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *
 }
 
 template <class E>
-bcf_status pagewise_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
-                           bool first_to_a, size_t n, size_t run_len, cudaStream_t s)
+bcf_status pagewise_rounds(const Call &c, const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
+                           bool first_to_a, size_t n, size_t run_len)
 {
     const void *ksrc = k0;
     const uint32_t *vsrc = v0;
@@ -509,7 +283,7 @@ bcf_status pagewise_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_
     for (size_t l = run_len; l < n; l *= 2) {
         void *kd = to_a ? ka : kb;
         uint32_t *vd = to_a ? va : vb;
-        bcf_status st = launch_pagewise<E>(ksrc, vsrc, kd, vd, n, l, s);
+        bcf_status st = launch_pagewise<E>(c, ksrc, vsrc, kd, vd, n, l);
         if (st != BCF_OK) return st;
         ksrc = kd;
         vsrc = vd;
@@ -520,10 +294,11 @@ bcf_status pagewise_rounds(const void *k0, const uint32_t *v0, void *ka, uint32_
 
 bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d_vals_in, void *d_keys_out,
                              void *d_vals_out, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
-                             void *d_workspace, size_t workspace_bytes, cudaStream_t s)
+                             void *d_workspace, size_t workspace_bytes, cudaStream_t s, const bcf_options *options)
 {
-    ProfileGroup profile_group(s);
-    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
+    Call c;
+    c.s = s;
+    if (!valid_types(kt, vt) || !resolve_options(options, &c.opt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
     if (!d_keys_in || !d_keys_out) return BCF_ERR_INVALID_ARG;
@@ -541,30 +316,125 @@ bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d
     if (overlap(d_workspace, need, d_keys_in, kb) || overlap(d_workspace, need, d_keys_out, kb) ||
         overlap(d_workspace, need, d_vals_in, vb) || overlap(d_workspace, need, d_vals_out, vb))
         return BCF_ERR_INVALID_ARG;
-    bcf_status st = check_device();
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
+    resolve_launch_mode(&c.opt, n);
+    ProfileGroup profile_group(s);
 
     const size_t runs = (n + run_len - 1) / run_len;
     const int rounds = ceil_log2(runs);
     if (rounds == 0) {   // a single run: the result is the input
-        if (cudaMemcpyAsync(d_keys_out, d_keys_in, kb, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BCF_ERR_CUDA;
-        if (vb && cudaMemcpyAsync(d_vals_out, d_vals_in, vb, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BCF_ERR_CUDA;
+        BCF_CUDA(cudaMemcpyAsync(d_keys_out, d_keys_in, kb, cudaMemcpyDeviceToDevice, s));
+        if (vb) BCF_CUDA(cudaMemcpyAsync(d_vals_out, d_vals_in, vb, cudaMemcpyDeviceToDevice, s));
         return BCF_OK;
     }
     // pass i (1-based) writes to `out` when (passes - i) is even, so the last pass lands in out.
-    const int passes = pagewise ? rounds : count_passes(n, run_len, kt, vt);
-    const Workspace w = carve(d_workspace, n, kt, vt, passes >= 2, pagewise ? 0 : max_shares(n, run_len));
+    const int passes = pagewise ? rounds : count_passes(n, run_len, n, kt, vt, c.opt);
+    const Workspace w = carve(d_workspace, n, kt, vt, rounds >= 2, pagewise ? 0 : max_shares(n, run_len));
     const bool first_to_out = ((passes - 1) % 2 == 0);
     if (pagewise) {
-        BCF_DISPATCH(kt, vt, st = pagewise_rounds<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
+        BCF_DISPATCH(kt, vt, st = pagewise_rounds<E>(c, d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
                                                      static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out,
-                                                     n, run_len, s));
+                                                     n, run_len));
     } else {
-        BCF_DISPATCH(kt, vt, st = merge_rounds<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
+        BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
                                                   static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out, n,
-                                                  run_len, w.splits, s));
+                                                  run_len, n, w.splits));
     }
     return st;
+}
+
+// base case of bcf_sort under `o` for an element type: the network and the length of the runs it leaves
+void resolve_base_case(const Opt &o, bcf_key_t kt, bcf_val_t vt, int *bc, size_t *base_run)
+{
+    // AUTO: what measures fastest on B200 -- long tiles for 4-byte keys alone, the tile mergesort otherwise
+    *bc = o.base_case;
+    if (*bc == BCF_BASE_AUTO) *bc = (kt == BCF_KEY_U32 && vt == BCF_VAL_NONE) ? BCF_BASE_LONG_TILES : BCF_BASE_TILE_MERGESORT;
+    *base_run = (*bc == BCF_BASE_LONG_TILES) ? size_t(BCF_LONG_TILE_H) * TILE : size_t(TILE);
+}
+
+// Base case + merge passes until runs of at least stop_len (stop_len >= n: the whole sort), in place: the
+// result is in d_keys / d_vals.  Validation is the caller's.
+bcf_status sort_phases(const Call &c, void *d_keys, void *d_vals, size_t n, size_t stop_len, bcf_key_t kt, bcf_val_t vt,
+                       void *d_workspace)
+{
+    int bc;
+    size_t base_run;
+    resolve_base_case(c.opt, kt, vt, &bc, &base_run);
+    const int passes = n > base_run ? count_passes(n, base_run, stop_len, kt, vt, c.opt) : 0;
+    const Workspace w = carve(d_workspace, n, kt, vt, n > TILE, n > TILE ? max_shares(n, TILE) : 0);
+    uint32_t *vals = static_cast<uint32_t *>(d_vals);
+    // With an odd number of merge passes the base case writes into the workspace, so that the
+    // last pass lands in the caller's buffer without an extra copy.
+    const bool base_to_ws = (passes % 2 == 1);
+    void *k0 = base_to_ws ? w.keys : d_keys;
+    uint32_t *v0 = base_to_ws ? w.vals : vals;
+    bcf_status st;
+    if (bc == BCF_BASE_LONG_TILES)
+        BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(c, d_keys, vals, k0, v0, n, BCF_LONG_TILE_H));
+    else
+        BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(c, d_keys, vals, k0, v0, n, bc));
+    if (st != BCF_OK || passes == 0) return st;
+    // pass 1 writes to the buffer the base case did not write.
+    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, base_run,
+                                              stop_len, w.splits));
+    return st;
+}
+
+bcf_status validate_sort(const void *d_keys, const void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, const void *d_workspace,
+                         size_t workspace_bytes)
+{
+    if (n >= (size_t(1) << 32)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys) || !aligned16(d_vals) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    const size_t need = bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt);
+    if (need && (!d_workspace || workspace_bytes < need)) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
+    if (overlap(d_workspace, need, d_keys, kb) || overlap(d_workspace, need, d_vals, vb)) return BCF_ERR_INVALID_ARG;
+    return BCF_OK;
+}
+
+// ------------------------------------------------------------------ FIND-BUCKETS and the final merge phase
+
+bool buckets_geom(size_t n, size_t run_len, int t, int P, int pivot_buckets, BucketsGeom *g)
+{
+    if (n == 0 || n >= (size_t(1) << 32) || run_len == 0 || t < 1 || P < 2) return false;
+    const size_t s = (n + run_len - 1) / run_len;
+    if (s > 65536 || (size_t)t > 65536 || (size_t)P > 65536 || s * (size_t)t < (size_t)P) return false;
+    g->n = n; g->run_len = run_len;
+    g->s = (unsigned)s; g->t = (unsigned)t; g->P = (unsigned)P;
+    g->pb = pivot_buckets ? 1 : 0;
+    g->nb = pivot_buckets ? 2u * P - 1u : (unsigned)P;
+    return (size_t)g->nb * s < (size_t(1) << 26);
+}
+
+bcf_status find_buckets_impl(const Call &c, const void *d_keys_in, const BucketsGeom &g, bcf_key_t kt, void *d_keys_out,
+                             void *d_pivots, uint32_t *d_piece_offsets, void *d_workspace)
+{
+    const size_t ns = (size_t)g.s * g.t;
+    char *ws = static_cast<char *>(d_workspace);
+    void *samples = ws;
+    uint32_t *bounds = reinterpret_cast<uint32_t *>(ws + align_up(ns * key_bytes(kt), 256));
+    char *sort_ws = reinterpret_cast<char *>(bounds) + align_up((size_t)g.s * (g.nb + 1) * 4, 256);
+    bcf_status st = launch_buckets_sample(c, d_keys_in, samples, g, kt);                      // Alg. 7
+    if (st != BCF_OK) return st;
+    st = sort_phases(c, samples, nullptr, ns, ns, kt, BCF_VAL_NONE, sort_ws);                  // MERGESORT(S), L505
+    if (st != BCF_OK) return st;
+    return launch_buckets_distribute(c, d_keys_in, samples, d_pivots, bounds, d_piece_offsets, d_keys_out, g, kt);
+}
+
+// pairs of the first round of the final merge phase (the round with the most pairs)
+inline size_t pieces_max_pairs(size_t groups, size_t s) { return groups * ((s + 1) / 2); }
+
+// Every kernel the library can launch, by bcf_kernel_id (each translation unit knows its own).
+template <class E>
+bool kernel_desc(int id, bcf_key_t kt, KernelDesc *k)
+{
+    if (kernel_desc_tile<E>(id, k) || kernel_desc_long<E>(id, k) || kernel_desc_merge<E>(id, k) || kernel_desc_pipe<E>(id, k) ||
+        kernel_desc_merge4<E>(id, k))
+        return true;
+    if constexpr (!E::HAS_VAL) return kernel_desc_pieces(id, kt, k);
+    return false;
 }
 
 }  // namespace
@@ -586,7 +456,21 @@ const char *bcf_status_string(bcf_status s)
     return "BCF_ERR_UNKNOWN";
 }
 
-const char *bcf_version(void) { return "bcf 0.1 (sm_100a)"; }
+const char *bcf_version(void) { return "bcf 0.2 (sm_100a)"; }
+
+bcf_status bcf_options_init(bcf_options *opt)
+{
+    if (!opt) return BCF_ERR_INVALID_ARG;
+    opt->struct_size = sizeof(bcf_options);
+    opt->base_case = BCF_BASE_AUTO;
+    opt->rounds_per_pass = 0;
+    opt->merge_impl = BCF_MERGE_IMPL_AUTO;
+    opt->partition_warp_search_max = -1;
+    opt->launch_mode = BCF_LAUNCH_AUTO;
+    return BCF_OK;
+}
+
+int bcf_last_cuda_error(void) { return last_cuda_error_ref(); }
 
 size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
 {
@@ -598,7 +482,7 @@ size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_v
         if (run_len == 0) return 0;
         const int rounds = ceil_log2((n + run_len - 1) / run_len);
         if (rounds == 0) return 0;
-        return carve(nullptr, n, kt, vt, count_passes(n, run_len, kt, vt) >= 2, max_shares(n, run_len)).bytes;
+        return carve(nullptr, n, kt, vt, rounds >= 2, max_shares(n, run_len)).bytes;   // whatever the options
     }
     case BCF_OP_MERGE_PAGEWISE: {
         if (run_len == 0) return 0;
@@ -620,16 +504,19 @@ size_t bcf_workspace_bytes(int op, size_t n, size_t run_len, bcf_key_t kt, bcf_v
 static bcf_status sort_tiles_common(void *d_keys, void *d_vals, size_t num_tiles, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream,
                                     int algo)
 {
-    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (num_tiles == 0) return BCF_OK;
     if (num_tiles >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
     if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_keys) || !aligned16(d_vals)) return BCF_ERR_MISALIGNED;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
-    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, static_cast<uint32_t *>(d_vals), d_keys,
-                                                  static_cast<uint32_t *>(d_vals), num_tiles * TILE, stream, algo));
+    ProfileGroup profile_group(stream);
+    BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(c, d_keys, static_cast<uint32_t *>(d_vals), d_keys,
+                                                  static_cast<uint32_t *>(d_vals), num_tiles * TILE, algo));
     return st;
 }
 
@@ -647,32 +534,25 @@ bcf_status bcf_sort_tiles_mergesort(void *d_keys, void *d_vals, size_t num_tiles
 bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles, int h, bcf_key_t kt, bcf_val_t vt,
                                bcf_stream_t stream)
 {
-    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt) || (h != 2 && h != 4 && h != 8)) return BCF_ERR_INVALID_ARG;
     if (num_long_tiles == 0) return BCF_OK;
     if (num_long_tiles * h >= (size_t(1) << 22)) return BCF_ERR_INVALID_ARG;
     if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_keys) || !aligned16(d_vals)) return BCF_ERR_MISALIGNED;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
-    BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(d_keys, static_cast<uint32_t *>(d_vals), d_keys, static_cast<uint32_t *>(d_vals),
-                                                  num_long_tiles * h * TILE, h, stream));
+    ProfileGroup profile_group(stream);
+    BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(c, d_keys, static_cast<uint32_t *>(d_vals), d_keys, static_cast<uint32_t *>(d_vals),
+                                                  num_long_tiles * h * TILE, h));
     return st;
 }
-
-bcf_status bcf_set_base_case(int base)
-{
-    if (base < BCF_BASE_SHEARSORT || base > BCF_BASE_AUTO) return BCF_ERR_INVALID_ARG;
-    g_base_case = base;
-    return BCF_OK;
-}
-
-int bcf_get_base_case(void) { return base_case(); }
 
 bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
                                bcf_val_t vt, uint32_t *d_splits, size_t num_shares, bcf_stream_t stream)
 {
-    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
@@ -680,46 +560,41 @@ bcf_status bcf_merge_partition(const void *d_keys_in, const void *d_vals_in, siz
     if (!aligned16(d_keys_in) || !aligned16(d_vals_in)) return BCF_ERR_MISALIGNED;
     const PassGeom g = pass_geom(n, run_len);
     if (num_shares != g.num_shares) return BCF_ERR_INVALID_ARG;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
-    BCF_DISPATCH(kt, vt, st = launch_partition<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, g, stream));
+    ProfileGroup profile_group(stream);
+    BCF_DISPATCH(kt, vt, st = launch_partition<E>(c, d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, g));
     return st;
 }
 
 bcf_status bcf_merge_partition4(const void *d_keys_in, const void *d_vals_in, size_t n, size_t run_len, bcf_key_t kt,
                                 bcf_val_t vt, uint32_t *d_splits, size_t num_bounds, bcf_stream_t stream)
 {
-    ProfileGroup profile_group(stream);
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
     if (n >= (size_t(1) << 32) || run_len == 0) return BCF_ERR_INVALID_ARG;
     if (!d_keys_in || !d_splits || (vt == BCF_VAL_U32) != (d_vals_in != nullptr)) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_keys_in) || !aligned16(d_vals_in) || !aligned16(d_splits)) return BCF_ERR_MISALIGNED;
     if (num_bounds != (n + BCF_SHARE - 1) / BCF_SHARE + 1) return BCF_ERR_INVALID_ARG;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
-    BCF_DISPATCH(kt, vt, st = launch_partition4<E>(d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, n, run_len,
-                                                   num_bounds, stream));
+    ProfileGroup profile_group(stream);
+    BCF_DISPATCH(kt, vt, st = launch_partition4<E>(c, d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_splits, n, run_len,
+                                                   num_bounds));
     return st;
 }
 
 // ------------------------------------------------------------------ FIND-BUCKETS (Alg. 7)
 
-static bool buckets_geom(size_t n, size_t run_len, int t, int P, int pivot_buckets, buckets::Geom *g)
-{
-    if (n == 0 || n >= (size_t(1) << 32) || run_len == 0 || t < 1 || P < 2) return false;
-    const size_t s = (n + run_len - 1) / run_len;
-    if (s > 65536 || (size_t)t > 65536 || (size_t)P > 65536 || s * (size_t)t < (size_t)P) return false;
-    g->n = n; g->run_len = run_len;
-    g->s = (unsigned)s; g->t = (unsigned)t; g->P = (unsigned)P;
-    g->pb = pivot_buckets ? 1 : 0;
-    g->nb = pivot_buckets ? 2u * P - 1u : (unsigned)P;
-    return (size_t)g->nb * s < (size_t(1) << 26);
-}
-
 size_t bcf_find_buckets_workspace_bytes(size_t n, size_t run_len, int t, int P, int pivot_buckets, bcf_key_t kt)
 {
-    buckets::Geom g;
+    BucketsGeom g;
     if (!valid_types(kt, BCF_VAL_NONE) || !buckets_geom(n, run_len, t, P, pivot_buckets, &g)) return 0;
     const size_t st = (size_t)g.s * g.t;
     return align_up(st * key_bytes(kt), 256) + align_up((size_t)g.s * (g.nb + 1) * 4, 256) +
@@ -732,7 +607,7 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
 {
     if (!valid_types(kt, BCF_VAL_NONE)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
-    buckets::Geom g;
+    BucketsGeom g;
     if (!buckets_geom(n, run_len, t, P, pivot_buckets, &g)) return BCF_ERR_INVALID_ARG;
     if (!d_keys_in || !d_keys_out || !d_pivots || !d_piece_offsets || !d_workspace) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
@@ -741,109 +616,194 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
     const size_t need = bcf_find_buckets_workspace_bytes(n, run_len, t, P, pivot_buckets, kt);
     if (workspace_bytes < need) return BCF_ERR_WORKSPACE_TOO_SMALL;
     if (overlap(d_workspace, need, d_keys_in, kb) || overlap(d_workspace, need, d_keys_out, kb)) return BCF_ERR_INVALID_ARG;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
     ProfileGroup profile_group(stream);
+    return find_buckets_impl(c, d_keys_in, g, kt, d_keys_out, d_pivots, d_piece_offsets, d_workspace);
+}
 
-    const size_t ns = (size_t)g.s * g.t;
-    char *ws = static_cast<char *>(d_workspace);
-    void *samples = ws;
-    uint32_t *bounds = reinterpret_cast<uint32_t *>(ws + align_up(ns * key_bytes(kt), 256));
-    char *sort_ws = reinterpret_cast<char *>(bounds) + align_up((size_t)g.s * (g.nb + 1) * 4, 256);
-    const size_t sort_ws_bytes = workspace_bytes - static_cast<size_t>(sort_ws - ws);
-    const bool k64 = (kt == BCF_KEY_U64);
-    {
-        const unsigned blocks = static_cast<unsigned>((ns + 255) / 256);
-        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
-        if (k64) buckets::sample_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, samples, g);
-        else buckets::sample_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, samples, g);
-    }
-    if (cudaPeekAtLastError() != cudaSuccess) return BCF_ERR_CUDA;
-    st = bcf_sort(samples, nullptr, ns, kt, BCF_VAL_NONE, sort_ws, sort_ws_bytes, stream);   // MERGESORT(S)
+// ------------------------------------------------------------------ final merge phase, BCFMergesort(PB) end to end
+
+size_t bcf_merge_pieces_workspace_bytes(size_t n, size_t groups, size_t s, bcf_key_t kt)
+{
+    if (!valid_types(kt, BCF_VAL_NONE) || n == 0 || groups == 0 || s == 0) return 0;
+    const size_t tmp = ceil_log2(s) >= 2 ? align_up(n * key_bytes(kt), 256) : 0;
+    return tmp + align_up((pieces_max_pairs(groups, s) + 1) * 4, 256);
+}
+
+bcf_status bcf_merge_pieces(const void *d_keys_in, void *d_keys_out, size_t n, const uint32_t *d_piece_offsets, size_t groups,
+                            size_t s, int copy_odd_groups, bcf_key_t kt, void *d_workspace, size_t workspace_bytes,
+                            bcf_stream_t stream)
+{
+    if (!valid_types(kt, BCF_VAL_NONE)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || groups == 0 || s == 0 || s > 65536 || groups * s >= (size_t(1) << 26)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_keys_out || !d_piece_offsets || !d_workspace) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    const size_t kb = n * key_bytes(kt);
+    const size_t need = bcf_merge_pieces_workspace_bytes(n, groups, s, kt);
+    if (workspace_bytes < need) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    if (overlap(d_keys_in, kb, d_keys_out, kb) || overlap(d_workspace, need, d_keys_in, kb) ||
+        overlap(d_workspace, need, d_keys_out, kb))
+        return BCF_ERR_INVALID_ARG;
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
-    {
-        const size_t work = (size_t)g.s * (g.P - 1);
-        const unsigned blocks = static_cast<unsigned>((work + 127) / 128);
-        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
-        if (k64) buckets::rank_kernel<2><<<blocks, 128, 0, stream>>>(d_keys_in, samples, d_pivots, bounds, g);
-        else buckets::rank_kernel<1><<<blocks, 128, 0, stream>>>(d_keys_in, samples, d_pivots, bounds, g);
+    ProfileGroup profile_group(stream);
+    if (s == 1) {
+        BCF_CUDA(cudaMemcpyAsync(d_keys_out, d_keys_in, kb, cudaMemcpyDeviceToDevice, stream));
+        return BCF_OK;
     }
-    {
-        LaunchTimer tm(BCF_KERNEL_PARTITION, stream);
-        buckets::offsets_kernel<<<1, buckets::SCAN_THREADS, 0, stream>>>(bounds, d_piece_offsets, g);
+    char *ws = static_cast<char *>(d_workspace);
+    void *tmp = ws;
+    uint32_t *first = reinterpret_cast<uint32_t *>(ws + (ceil_log2(s) >= 2 ? align_up(kb, 256) : 0));
+    return launch_merge_pieces_rounds(c, d_keys_in, d_keys_out, tmp, n, d_piece_offsets, groups, s, copy_odd_groups, first, kt);
+}
+
+// run length at which the first merge phase is suspended: the first base_run * 2^r that leaves at most P runs
+static size_t buckets_stop_len(size_t n, size_t base_run, int P)
+{
+    size_t l = base_run;
+    while ((n + l - 1) / l > static_cast<size_t>(P)) l *= 2;
+    return l;
+}
+
+// [keys copy W1][piece offsets][pivots][max(sort workspace, FIND-BUCKETS workspace, final-phase workspace)]
+struct BucketsWs {
+    size_t w1, offsets, pivots, rest, total;
+};
+static BucketsWs buckets_ws(size_t n, int t, int P, int pb, bcf_key_t kt)
+{
+    BucketsWs w;
+    const size_t kb = align_up(n * key_bytes(kt), 256);
+    const size_t nb = pb ? 2 * size_t(P) - 1 : size_t(P);
+    w.w1 = 0;
+    w.offsets = kb;
+    w.pivots = w.offsets + align_up((nb * size_t(P) + 1) * 4, 256);
+    w.rest = w.pivots + align_up(size_t(P) * key_bytes(kt), 256);
+    size_t rest = bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, BCF_VAL_NONE);
+    // the distribution runs on s <= P runs of any of the run lengths a base case can leave
+    size_t fb = 0;
+    for (size_t base : {size_t(TILE), size_t(BCF_LONG_TILE_H) * TILE}) {
+        const size_t l = buckets_stop_len(n, base, P);
+        const size_t v = bcf_find_buckets_workspace_bytes(n, l, t, P, pb, kt);
+        if (v > fb) fb = v;
     }
-    {
-        const size_t chunks = ((run_len + buckets::SCATTER_CHUNK - 1) / buckets::SCATTER_CHUNK) * g.s;
-        const unsigned blocks = static_cast<unsigned>(chunks < 148 * 64 ? chunks : 148 * 64);
-        LaunchTimer tm(BCF_KERNEL_MERGE, stream);
-        if (k64) buckets::scatter_kernel<2><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
-        else buckets::scatter_kernel<1><<<blocks, 256, 0, stream>>>(d_keys_in, d_keys_out, bounds, d_piece_offsets, g);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+    if (fb > rest) rest = fb;
+    const size_t mp = bcf_merge_pieces_workspace_bytes(n, nb, size_t(P), kt);
+    if (mp > rest) rest = mp;
+    w.total = w.rest + align_up(rest, 256);
+    return w;
+}
+
+size_t bcf_sort_buckets_workspace_bytes(size_t n, int t, int P, int pivot_buckets, bcf_key_t kt)
+{
+    if (!valid_types(kt, BCF_VAL_NONE) || n == 0 || n >= (size_t(1) << 32) || t < 1 || t > 65536 || P < 2 || P > 65536) return 0;
+    return buckets_ws(n, t, P, pivot_buckets, kt).total;
+}
+
+bcf_status bcf_sort_buckets(void *d_keys, size_t n, bcf_key_t kt, int t, int P, int pivot_buckets, uint32_t *d_bucket_starts,
+                            void *d_workspace, size_t workspace_bytes, bcf_stream_t stream, const bcf_options *options)
+{
+    Call c;
+    c.s = stream;
+    if (!valid_types(kt, BCF_VAL_NONE) || !resolve_options(options, &c.opt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || t < 1 || t > 65536 || P < 2 || P > 65536) return BCF_ERR_INVALID_ARG;
+    if (!d_keys || !d_workspace) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    const BucketsWs w = buckets_ws(n, t, P, pivot_buckets, kt);
+    if (workspace_bytes < w.total) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    const size_t kb = n * key_bytes(kt);
+    if (overlap(d_workspace, w.total, d_keys, kb)) return BCF_ERR_INVALID_ARG;
+    bcf_status st = current_device(&c.dev);
+    if (st != BCF_OK) return st;
+    resolve_launch_mode(&c.opt, n);
+    ProfileGroup profile_group(stream);
+
+    char *ws = static_cast<char *>(d_workspace);
+    void *w1 = ws + w.w1;
+    uint32_t *offsets = reinterpret_cast<uint32_t *>(ws + w.offsets);
+    void *pivots = ws + w.pivots;
+    void *rest = ws + w.rest;
+
+    // phases 1 + 2: base case, merge rounds while more than P runs remain (result in d_keys).  The sort
+    // workspace of these phases is [W1 = the ping-pong copy][..]: carve() puts its keys copy first.
+    int bc;
+    size_t base_run;
+    resolve_base_case(c.opt, kt, BCF_VAL_NONE, &bc, &base_run);
+    const size_t stop_len = buckets_stop_len(n, base_run, P);
+    // the sort's own workspace layout (keys copy + splits) needs bcf_workspace_bytes(SORT) contiguous bytes:
+    // W1 followed by the offsets / pivots / rest regions covers it (they are written only after these phases)
+    st = sort_phases(c, d_keys, nullptr, n, stop_len, kt, BCF_VAL_NONE, d_workspace);
+    if (st != BCF_OK) return st;
+    const size_t s = (n + stop_len - 1) / stop_len;
+    if (s <= 1) return BCF_OK;
+
+    // phase 3: FIND-BUCKETS  d_keys -> W1
+    BucketsGeom g;
+    int tt = t;
+    if (s * static_cast<size_t>(tt) < static_cast<size_t>(P)) tt = static_cast<int>((P + s - 1) / s);   // s t >= P
+    if (!buckets_geom(n, stop_len, tt, P, pivot_buckets, &g)) return BCF_ERR_INVALID_ARG;
+    st = find_buckets_impl(c, d_keys, g, kt, w1, pivots, offsets, rest);
+    if (st != BCF_OK) return st;
+    if (d_bucket_starts)
+        BCF_CUDA(cudaMemcpy2DAsync(d_bucket_starts, 4, offsets, s * 4, 4, g.nb + 1, cudaMemcpyDeviceToDevice, stream));
+
+    // phase 4: the final merge phase inside the buckets  W1 -> d_keys
+    char *r = static_cast<char *>(rest);
+    const int rounds = ceil_log2(s);
+    void *tmp = r;
+    uint32_t *first = reinterpret_cast<uint32_t *>(r + (rounds >= 2 ? align_up(kb, 256) : 0));
+    return launch_merge_pieces_rounds(c, w1, d_keys, tmp, n, offsets, g.nb, s, pivot_buckets ? 1 : 0, first, kt);
 }
 
 // ------------------------------------------------------------------ coloured prefix sums (App. A)
 
-static unsigned colored_scan_grid(size_t n)
-{
-    const size_t pages = (n + cscan::PAGE - 1) / cscan::PAGE;
-    const size_t ctas = (pages + cscan::WARPS - 1) / cscan::WARPS;
-    return static_cast<unsigned>(ctas < 2048 ? ctas : 2048);
-}
-
 size_t bcf_colored_prefix_sums_workspace_bytes(size_t n)
 {
     if (n == 0) return 0;
-    return align_up(size_t(colored_scan_grid(n)) * cscan::WARPS * cscan::MAX_COLORS * 4, 256);
+    return colored_scan_workspace_bytes(n);
 }
 
 bcf_status bcf_colored_prefix_sums(const uint32_t *d_values, const uint8_t *d_colors, size_t n, int num_colors, int layout,
                                    uint32_t *d_out, void *d_workspace, size_t workspace_bytes, bcf_stream_t stream)
 {
     if (n == 0) return BCF_OK;
-    if (n >= (size_t(1) << 32) || num_colors < 1 || num_colors > cscan::MAX_COLORS) return BCF_ERR_INVALID_ARG;
+    if (n >= (size_t(1) << 32) || num_colors < 1 || num_colors > colored_scan_max_colors()) return BCF_ERR_INVALID_ARG;
     if (layout != BCF_SCAN_BANK_PER_THREAD && layout != BCF_SCAN_THREAD_MAJOR) return BCF_ERR_INVALID_ARG;
     if (!d_values || !d_colors || !d_out || !d_workspace) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_values) || !aligned16(d_colors) || !aligned16(d_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
     if (overlap(d_out, n * 4, d_values, n * 4) || overlap(d_out, n * 4, d_colors, n)) return BCF_ERR_INVALID_ARG;
     if (workspace_bytes < bcf_colored_prefix_sums_workspace_bytes(n)) return BCF_ERR_WORKSPACE_TOO_SMALL;
-    bcf_status st = check_device();
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    const bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
     ProfileGroup profile_group(stream);
-    const unsigned grid = colored_scan_grid(n);
-    const unsigned long long warps = static_cast<unsigned long long>(grid) * cscan::WARPS;
-    uint32_t *partial = static_cast<uint32_t *>(d_workspace);
-    const bool cf = (layout == BCF_SCAN_BANK_PER_THREAD);
-    {
-        LaunchTimer t(BCF_KERNEL_PARTITION, stream);
-        if (cf) cscan::reduce_kernel<true><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial);
-        else cscan::reduce_kernel<false><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial);
-    }
-    {
-        LaunchTimer t(BCF_KERNEL_PARTITION, stream);
-        cscan::offsets_kernel<<<1, cscan::MAX_COLORS * 32, 0, stream>>>(partial, warps, num_colors);
-    }
-    {
-        LaunchTimer t(BCF_KERNEL_MERGE, stream);
-        if (cf) cscan::scan_kernel<true><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial, d_out);
-        else cscan::scan_kernel<false><<<grid, cscan::WARPS * 32, 0, stream>>>(d_values, d_colors, n, num_colors, partial, d_out);
-    }
-    return cudaPeekAtLastError() == cudaSuccess ? BCF_OK : BCF_ERR_CUDA;
+    return launch_colored_scan(c, d_values, d_colors, n, num_colors, layout == BCF_SCAN_BANK_PER_THREAD,
+                               static_cast<uint32_t *>(d_workspace), d_out);
 }
 
-bcf_status bcf_set_rounds_per_pass(int rounds)
+int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt, const bcf_options *options)
 {
-    if (rounds != 1 && rounds != 2) return BCF_ERR_INVALID_ARG;
-    g_rounds_per_pass = rounds;
-    return BCF_OK;
+    Opt o;
+    if (!valid_types(kt, vt) || n == 0 || run_len == 0 || !resolve_options(options, &o)) return 0;
+    return count_passes(n, run_len, n, kt, vt, o);
 }
 
-int bcf_get_rounds_per_pass(void) { return rounds_per_pass(); }
-
-int bcf_merge_pass_count(size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt)
+bcf_status bcf_merge_runs_ex(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out, size_t n,
+                             size_t run_len, bcf_key_t kt, bcf_val_t vt, void *d_workspace, size_t workspace_bytes,
+                             bcf_stream_t stream, const bcf_options *opt)
 {
-    if (!valid_types(kt, vt) || n == 0 || run_len == 0) return 0;
-    return count_passes(n, run_len, kt, vt);
+    return merge_runs_common(false, d_keys_in, d_vals_in, d_keys_out, d_vals_out, n, run_len, kt, vt, d_workspace,
+                             workspace_bytes, stream, opt);
 }
 
 bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out, size_t n,
@@ -851,7 +811,7 @@ bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_
                           bcf_stream_t stream)
 {
     return merge_runs_common(false, d_keys_in, d_vals_in, d_keys_out, d_vals_out, n, run_len, kt, vt, d_workspace,
-                             workspace_bytes, stream);
+                             workspace_bytes, stream, nullptr);
 }
 
 bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
@@ -859,51 +819,32 @@ bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in,
                                    size_t workspace_bytes, bcf_stream_t stream)
 {
     return merge_runs_common(true, d_keys_in, d_vals_in, d_keys_out, d_vals_out, n, run_len, kt, vt, d_workspace,
-                             workspace_bytes, stream);
+                             workspace_bytes, stream, nullptr);
+}
+
+bcf_status bcf_sort_ex(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_workspace,
+                       size_t workspace_bytes, bcf_stream_t stream, const bcf_options *options)
+{
+    Call c;
+    c.s = stream;
+    if (!valid_types(kt, vt) || !resolve_options(options, &c.opt)) return BCF_ERR_INVALID_ARG;
+    if (n == 0) return BCF_OK;
+    bcf_status st = validate_sort(d_keys, d_vals, n, kt, vt, d_workspace, workspace_bytes);
+    if (st != BCF_OK) return st;
+    if ((st = current_device(&c.dev)) != BCF_OK) return st;
+    resolve_launch_mode(&c.opt, n);
+    ProfileGroup profile_group(stream);
+    return sort_phases(c, d_keys, d_vals, n, n, kt, vt, d_workspace);
 }
 
 bcf_status bcf_sort(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_workspace,
                     size_t workspace_bytes, bcf_stream_t stream)
 {
-    ProfileGroup profile_group(stream);
-    if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
-    if (n == 0) return BCF_OK;
-    if (n >= (size_t(1) << 32)) return BCF_ERR_INVALID_ARG;
-    if (!d_keys || (vt == BCF_VAL_U32) != (d_vals != nullptr)) return BCF_ERR_INVALID_ARG;
-    if (!aligned16(d_keys) || !aligned16(d_vals) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
-    const size_t need = bcf_workspace_bytes(BCF_OP_SORT, n, 0, kt, vt);
-    if (need && (!d_workspace || workspace_bytes < need)) return BCF_ERR_WORKSPACE_TOO_SMALL;
-    const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
-    if (overlap(d_workspace, need, d_keys, kb) || overlap(d_workspace, need, d_vals, vb)) return BCF_ERR_INVALID_ARG;
-    bcf_status st = check_device();
-    if (st != BCF_OK) return st;
-
-    // base case: runs of base_run sorted elements (one tile, or a long tile of h tiles)
-    // AUTO: what measures fastest on B200 -- long tiles for 4-byte keys alone, the tile mergesort otherwise
-    int bc = base_case();
-    if (bc == BCF_BASE_AUTO) bc = (kt == BCF_KEY_U32 && vt == BCF_VAL_NONE) ? BCF_BASE_LONG_TILES : BCF_BASE_TILE_MERGESORT;
-    const size_t base_run = (bc == BCF_BASE_LONG_TILES) ? size_t(BCF_LONG_TILE_H) * TILE : size_t(TILE);
-    const int passes = n > base_run ? count_passes(n, base_run, kt, vt) : 0;
-    const Workspace w = carve(d_workspace, n, kt, vt, passes > 0, passes > 0 ? max_shares(n, TILE) : 0);
-    uint32_t *vals = static_cast<uint32_t *>(d_vals);
-    // With an odd number of merge passes the base case writes into the workspace, so that the
-    // last pass lands in the caller's buffer without an extra copy.
-    const bool base_to_ws = (passes % 2 == 1);
-    void *k0 = base_to_ws ? w.keys : d_keys;
-    uint32_t *v0 = base_to_ws ? w.vals : vals;
-    if (bc == BCF_BASE_LONG_TILES)
-        BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(d_keys, vals, k0, v0, n, BCF_LONG_TILE_H, stream));
-    else
-        BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(d_keys, vals, k0, v0, n, stream, bc));
-    if (st != BCF_OK || passes == 0) return st;
-    // pass 1 writes to the buffer the base case did not write.
-    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, base_run,
-                                              w.splits, stream));
-    return st;
+    return bcf_sort_ex(d_keys, d_vals, n, kt, vt, d_workspace, workspace_bytes, stream, nullptr);
 }
 
-bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_scratch,
-                         size_t scratch_bytes, bcf_stream_t stream)
+bcf_status bcf_sort_host_ex(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_scratch,
+                            size_t scratch_bytes, bcf_stream_t stream, const bcf_options *options)
 {
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
     if (n == 0) return BCF_OK;
@@ -912,19 +853,26 @@ bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf
     if (!aligned16(d_scratch)) return BCF_ERR_MISALIGNED;
     const size_t need = bcf_workspace_bytes(BCF_OP_SORT_HOST, n, 0, kt, vt);
     if (!d_scratch || scratch_bytes < need) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    (void)cudaGetLastError();
     const size_t kb = n * key_bytes(kt), vb = (vt == BCF_VAL_U32) ? n * 4 : 0;
     char *base = static_cast<char *>(d_scratch);
     void *dk = base;
     void *dv = vb ? base + align_up(kb, 256) : nullptr;
     const size_t data = align_up(kb, 256) + (vb ? align_up(vb, 256) : 0);
-    if (cudaMemcpyAsync(dk, h_keys, kb, cudaMemcpyHostToDevice, stream) != cudaSuccess) return BCF_ERR_CUDA;
-    if (vb && cudaMemcpyAsync(dv, h_vals, vb, cudaMemcpyHostToDevice, stream) != cudaSuccess) return BCF_ERR_CUDA;
-    const bcf_status st = bcf_sort(dk, dv, n, kt, vt, base + data, scratch_bytes - data, stream);
+    BCF_CUDA(cudaMemcpyAsync(dk, h_keys, kb, cudaMemcpyHostToDevice, stream));
+    if (vb) BCF_CUDA(cudaMemcpyAsync(dv, h_vals, vb, cudaMemcpyHostToDevice, stream));
+    const bcf_status st = bcf_sort_ex(dk, dv, n, kt, vt, base + data, scratch_bytes - data, stream, options);
     if (st != BCF_OK) return st;
-    if (cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream) != cudaSuccess) return BCF_ERR_CUDA;
-    if (vb && cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream) != cudaSuccess) return BCF_ERR_CUDA;
-    if (cudaStreamSynchronize(stream) != cudaSuccess) return BCF_ERR_CUDA;
+    BCF_CUDA(cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream));
+    if (vb) BCF_CUDA(cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream));
+    BCF_CUDA(cudaStreamSynchronize(stream));
     return BCF_OK;
+}
+
+bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf_val_t vt, void *d_scratch,
+                         size_t scratch_bytes, bcf_stream_t stream)
+{
+    return bcf_sort_host_ex(h_keys, h_vals, n, kt, vt, d_scratch, scratch_bytes, stream, nullptr);
 }
 
 // ------------------------------------------------------------------ measurement hooks
@@ -934,6 +882,7 @@ bcf_status bcf_profile_enable(int on)
     g_prof.on = on != 0;
     g_prof.used = 0;
     g_prof.open_since = -1;
+    g_prof.dropped = 0;
     return BCF_OK;
 }
 
@@ -953,6 +902,8 @@ bcf_status bcf_profile_read(float *ms, unsigned long long *launches)
     return BCF_OK;
 }
 
+unsigned long long bcf_profile_dropped(void) { return g_prof.dropped; }
+
 void bcf_launch_counts(unsigned long long *launches)
 {
     for (int c = 0; c < BCF_KERNEL_CLASSES; ++c) {
@@ -961,33 +912,33 @@ void bcf_launch_counts(unsigned long long *launches)
     }
 }
 
-bcf_status bcf_kernel_info(int kernel_class, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread, int *smem_bytes_per_cta,
+const char *bcf_kernel_name(int kernel_id)
+{
+    static const char *names[BCF_KID_COUNT] = {
+        "tile_sort_kernel", "tile_mergesort_kernel", "long_tile_sort_kernel<h=2>", "long_tile_sort_kernel<h=4>",
+        "long_tile_sort_kernel<h=8>", "partition_kernel", "merge_kernel", "partition_share_kernel<G=1>",
+        "partition_share_kernel<G=32>", "merge_pipe_kernel", "partition4_kernel", "merge4_pipe_kernel",
+        "pagewise_merge_kernel", "merge_pieces_kernel"};
+    return (kernel_id >= 0 && kernel_id < BCF_KID_COUNT) ? names[kernel_id] : nullptr;
+}
+
+bcf_status bcf_kernel_info(int kernel_id, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread, int *smem_bytes_per_cta,
                            int *threads_per_cta, int *ctas_per_sm, int *local_bytes_per_thread)
 {
     if (!valid_types(kt, vt)) return BCF_ERR_INVALID_ARG;
-    const void *fn = nullptr;
-    size_t smem = 0;
-    int threads = WARPS_PER_CTA * 32;
-    BCF_DISPATCH(kt, vt, {
-        switch (kernel_class) {
-        case BCF_KERNEL_TILE_SORT: fn = (const void *)tile_sort_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
-        case BCF_KERNEL_TILE_MERGESORT: fn = (const void *)tile_mergesort_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
-        case BCF_KERNEL_PARTITION: fn = (const void *)partition_kernel<E>; smem = 0; threads = 128; break;
-        case BCF_KERNEL_MERGE: fn = (const void *)merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
-        case BCF_KERNEL_MERGE_PAGEWISE: fn = (const void *)pagewise_merge_kernel<E>; smem = WARPS_PER_CTA * warp_smem_bytes<E>(); break;
-        default: break;
-        }
-    });
-    if (!fn) return BCF_ERR_INVALID_ARG;
+    KernelDesc k = {nullptr, 0, 0};
+    bool ok = false;
+    BCF_DISPATCH(kt, vt, ok = kernel_desc<E>(kernel_id, kt, &k));
+    if (!ok || !k.fn) return BCF_ERR_INVALID_ARG;
+    (void)cudaGetLastError();
     cudaFuncAttributes a;
-    if (cudaFuncGetAttributes(&a, fn) != cudaSuccess) return BCF_ERR_CUDA;
-    if (smem > 48 * 1024 && cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-        return BCF_ERR_CUDA;
+    BCF_CUDA(cudaFuncGetAttributes(&a, k.fn));
+    if (k.smem > 48 * 1024) BCF_CUDA(cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem));
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem) != cudaSuccess) return BCF_ERR_CUDA;
+    BCF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k.fn, k.threads, k.smem));
     if (regs_per_thread) *regs_per_thread = a.numRegs;
-    if (smem_bytes_per_cta) *smem_bytes_per_cta = static_cast<int>(a.sharedSizeBytes + smem);
-    if (threads_per_cta) *threads_per_cta = threads;
+    if (smem_bytes_per_cta) *smem_bytes_per_cta = static_cast<int>(a.sharedSizeBytes + k.smem);
+    if (threads_per_cta) *threads_per_cta = k.threads;
     if (ctas_per_sm) *ctas_per_sm = occ;
     if (local_bytes_per_thread) *local_bytes_per_thread = static_cast<int>(a.localSizeBytes);
     return BCF_OK;

@@ -24,14 +24,7 @@ struct KeyT { using type = uint32_t; };
 template <>
 struct KeyT<2> { using type = unsigned long long; };
 
-struct Geom {
-    unsigned long long n, run_len;
-    unsigned int s;        // runs
-    unsigned int t;        // samples per run
-    unsigned int P;        // buckets without pivot buckets
-    unsigned int nb;       // buckets: P or 2P - 1
-    int pb;
-};
+using Geom = BucketsGeom;      // bcf_layout.cuh
 
 __device__ __forceinline__ unsigned long long run_length(const Geom &g, const unsigned int r)
 {
@@ -43,6 +36,7 @@ __device__ __forceinline__ unsigned long long run_length(const Geom &g, const un
 template <int KW>
 __global__ void sample_kernel(const void *__restrict__ kin, void *__restrict__ samples, const Geom g)
 {
+    pdl_entry();
     using K = typename KeyT<KW>::type;
     const unsigned long long id = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (id >= static_cast<unsigned long long>(g.s) * g.t) return;
@@ -58,6 +52,7 @@ template <int KW>
 __global__ void rank_kernel(const void *__restrict__ kin, const void *__restrict__ sorted_samples, void *__restrict__ pivots,
                             uint32_t *__restrict__ bounds, const Geom g)
 {
+    pdl_entry();
     using K = typename KeyT<KW>::type;
     const unsigned long long id = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     const unsigned int np = g.P - 1;
@@ -98,6 +93,7 @@ constexpr int SCAN_THREADS = 1024;
 __global__ void __launch_bounds__(SCAN_THREADS)
 offsets_kernel(const uint32_t *__restrict__ bounds, uint32_t *__restrict__ Q, const Geom g)
 {
+    pdl_entry();
     __shared__ unsigned long long sums[SCAN_THREADS];
     const unsigned long long total = static_cast<unsigned long long>(g.nb) * g.s;
     const unsigned long long chunk = (total + SCAN_THREADS - 1) / SCAN_THREADS;
@@ -136,6 +132,7 @@ __global__ void __launch_bounds__(256)
 scatter_kernel(const void *__restrict__ kin, void *__restrict__ kout, const uint32_t *__restrict__ bounds,
                const uint32_t *__restrict__ Q, const Geom g)
 {
+    pdl_entry();
     using K = typename KeyT<KW>::type;
     const unsigned long long chunks_per_run = (g.run_len + SCATTER_CHUNK - 1) / SCATTER_CHUNK;
     const unsigned long long total = chunks_per_run * g.s;

@@ -96,6 +96,7 @@ __global__ void __launch_bounds__(WARPS * 32)
 reduce_kernel(const uint32_t *__restrict__ vals, const unsigned char *__restrict__ cols, const unsigned long long n,
               const int d, uint32_t *__restrict__ partial)
 {
+    pdl_entry();
     __shared__ uint32_t sm[WARPS * MAX_COLORS * 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t *s = sm + warp * (MAX_COLORS * 32);
@@ -122,6 +123,7 @@ reduce_kernel(const uint32_t *__restrict__ vals, const unsigned char *__restrict
 __global__ void __launch_bounds__(MAX_COLORS * 32)
 offsets_kernel(uint32_t *__restrict__ partial, const unsigned long long num_warps, const int d)
 {
+    pdl_entry();
     const int lane = threadIdx.x & 31, c = threadIdx.x >> 5;
     if (c >= d) return;
     uint32_t carry = 0;
@@ -140,6 +142,7 @@ __global__ void __launch_bounds__(WARPS * 32)
 scan_kernel(const uint32_t *__restrict__ vals, const unsigned char *__restrict__ cols, const unsigned long long n, const int d,
             const uint32_t *__restrict__ offsets, uint32_t *__restrict__ out)
 {
+    pdl_entry();
     __shared__ uint32_t sm[WARPS * MAX_COLORS * 32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t *s = sm + warp * (MAX_COLORS * 32);

@@ -20,13 +20,25 @@
 
 namespace bcf {
 
-template <int KW, bool HV>
-struct Elem {
-    static constexpr int KEY_WORDS = KW;           // 1: u32 key, 2: u64 key
-    static constexpr bool HAS_VAL = HV;
-    static constexpr int NP = KW + (HV ? 1 : 0);   // planes
-    static constexpr int KEY_BYTES = 4 * KW;
-};
+// struct Elem<KEY_WORDS, HAS_VAL>: bcf_layout.cuh
+
+// ------------------------------------------------------------------ programmatic dependent launch
+// Every kernel of the library starts with pdl_entry(): it waits until the grids it depends on have completed and
+// their writes are visible (griddepcontrol.wait) -- before its first access to global memory.  With the launch
+// attribute (bcf_options.launch_mode = BCF_LAUNCH_PDL) the kernel's CTAs are scheduled as soon as the CTAs of
+// its predecessor have exited, so the launch latency overlaps the predecessor's drain; without it the
+// instruction does nothing.  No kernel triggers its dependents early (griddepcontrol.launch_dependents):
+// measured on B200, dependents that sit on the SMs while a merge pass runs slow it down.
+#ifndef BCF_PDL_EARLY_TRIGGER
+#define BCF_PDL_EARLY_TRIGGER 0
+#endif
+__device__ __forceinline__ void pdl_entry()
+{
+#if BCF_PDL_EARLY_TRIGGER
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
 
 // ------------------------------------------------------------------ compare-exchange
 //
@@ -36,8 +48,8 @@ struct Elem {
 // of the "larger" outputs are formed as  hi = a + b - lo  (mod 2^32, exact) with two IMADs whose
 // multiplier comes from constant memory -- opaque to ptxas, which would otherwise turn them back
 // into ALU adds.
-__constant__ uint32_t c_one = 1u;
-__constant__ uint32_t c_minus_one = 0xFFFFFFFFu;
+static __constant__ uint32_t c_one = 1u;            // one copy per translation unit
+static __constant__ uint32_t c_minus_one = 0xFFFFFFFFu;
 
 // a + b - lo on the FMA pipe (lo is one of a, b; the result is the other one).
 __device__ __forceinline__ uint32_t other_of(const uint32_t a, const uint32_t b, const uint32_t lo)
@@ -222,12 +234,7 @@ __device__ __forceinline__ void col_store(uint32_t *pl, const uint32_t (&v)[32],
 // position 32 k + c of the bitonic sequence P || reverse(Q): rows of P as they are, the rows of Q
 // in reverse order and mirrored (column 31 - c).  For a fixed k the 32 threads read the 32 words of
 // ONE row in a permuted order -> 32 distinct banks, like col_load.
-BCF_HD constexpr int merge_level_row(int T, int k)
-{
-    const int size = 1 << T, half = size >> 1, i = k & (size - 1);
-    return i < half ? k : (k - i) + half + (size - 1 - i);
-}
-BCF_HD constexpr bool merge_level_mirror(int T, int k) { return (k & ((1 << T) - 1)) >= (1 << (T - 1)); }
+// merge_level_row / merge_level_mirror: bcf_layout.cuh
 
 template <int T>
 __device__ __forceinline__ void col_load_level(const uint32_t *pl, uint32_t (&v)[32], const int c)

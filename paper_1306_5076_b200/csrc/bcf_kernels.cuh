@@ -237,6 +237,7 @@ template <class E>
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32)
 tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
 {
+    pdl_entry();
     extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -317,6 +318,7 @@ template <class E>
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32, E::NP == 1 ? BCF_TMS_MINB1 : E::NP == 2 ? BCF_TMS_MINB2 : BCF_TMS_MINB3)
 tile_mergesort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
 {
+    pdl_entry();
     extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -342,12 +344,7 @@ tile_mergesort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
 
 // ------------------------------------------------------------------ a5: merge partitioning
 
-struct PassGeom {
-    unsigned long long n;         // elements
-    unsigned long long run_len;   // L
-    unsigned int shares_per_pair; // ceil(2L / 1024)
-    unsigned long long num_shares;
-};
+// struct PassGeom: bcf_layout.cuh
 
 template <class E>
 __device__ __forceinline__ bool elem_le_global(const void *keys, const uint32_t *vals, const size_t ia, const size_t ib)
@@ -380,6 +377,7 @@ __global__ void __launch_bounds__(128)
 partition_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
                  uint32_t *__restrict__ splits, const PassGeom g)
 {
+    pdl_entry();
     const unsigned long long slot = static_cast<unsigned long long>(blockIdx.x) * blockDim.x + threadIdx.x;
     if (slot >= g.num_shares) return;
     const unsigned long long pair = slot / g.shares_per_pair;
@@ -418,6 +416,7 @@ merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
              void *__restrict__ kout, uint32_t *__restrict__ vout,
              const uint32_t *__restrict__ splits, const PassGeom g)
 {
+    pdl_entry();
     extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;

@@ -45,4 +45,42 @@ BCF_HD constexpr int elem_word(int r, int c) { return chunk_word(r, c >> 2) + (c
 // being written back-to-front).
 BCF_HD constexpr int mirrored_col(int k, int c) { return (k & 1) ? (31 - c) : c; }
 
+// Column sweep of the tile mergesort at level T (bcf_core.cuh col_load_level): register k of the thread of
+// column c holds position 32 k + c of P || reverse(Q) of its block of 2^T rows -- which row, and mirrored or not.
+BCF_HD constexpr int merge_level_row(int T, int k)
+{
+    const int size = 1 << T, half = size >> 1, i = k & (size - 1);
+    return i < half ? k : (k - i) + half + (size - 1 - i);
+}
+BCF_HD constexpr bool merge_level_mirror(int T, int k) { return (k & ((1 << T) - 1)) >= (1 << (T - 1)); }
+
+// ------------------------------------------------------------------ plain types shared by host and device code
+
+// An element is NP 32-bit "planes" compared lexicographically in plane order (bcf_core.cuh).
+template <int KW, bool HV>
+struct Elem {
+    static constexpr int KEY_WORDS = KW;           // 1: u32 key, 2: u64 key
+    static constexpr bool HAS_VAL = HV;
+    static constexpr int NP = KW + (HV ? 1 : 0);   // planes
+    static constexpr int KEY_BYTES = 4 * KW;
+};
+
+// geometry of one merge round of the one-warp-per-page kernels (bcf_kernels.cuh)
+struct PassGeom {
+    unsigned long long n;         // elements
+    unsigned long long run_len;   // L
+    unsigned int shares_per_pair; // ceil(2L / 1024)
+    unsigned long long num_shares;
+};
+
+// geometry of FIND-BUCKETS (bcf_buckets.cuh)
+struct BucketsGeom {
+    unsigned long long n, run_len;
+    unsigned int s;        // runs
+    unsigned int t;        // samples per run
+    unsigned int P;        // buckets without pivot buckets
+    unsigned int nb;       // buckets: P or 2P - 1
+    int pb;
+};
+
 }  // namespace bcf

@@ -117,6 +117,7 @@ template <class E, int H>
 __global__ void __launch_bounds__(H * 32, LongTileCfg<E, H>::min_ctas)
 long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, const size_t n)
 {
+    pdl_entry();
     extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -124,12 +125,15 @@ long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
     // A warp's working planes (transposes inside its tile) are its own slot of the set the NEXT stage
     // writes: its last readers passed a barrier since.
     uint32_t *const slot = smem + warp * (E::NP * TILE);
-    const size_t num_tiles = (n + TILE - 1) / TILE;
-    const size_t num_groups = (num_tiles + H - 1) / H;
+    // 32-bit group / tile counters (n < 2^32): fewer live registers in the loop than size_t arithmetic
+    const unsigned num_tiles = static_cast<unsigned>((n + TILE - 1) / TILE);
+    const unsigned num_groups = (num_tiles + H - 1) / H;
+    const unsigned full_tiles = static_cast<unsigned>(n / TILE);
 
-    for (size_t g = blockIdx.x; g < num_groups; g += gridDim.x) {
-        const size_t base = (g * H + warp) * TILE;
-        const int cnt = base >= n ? 0 : ((n - base) < static_cast<size_t>(TILE) ? static_cast<int>(n - base) : TILE);
+    for (unsigned g = blockIdx.x; g < num_groups; g += gridDim.x) {
+        const unsigned tile = g * H + warp;
+        const size_t base = static_cast<size_t>(tile) * TILE;
+        const int cnt = tile < full_tiles ? TILE : (tile < num_tiles ? static_cast<int>(n - base) : 0);
         uint32_t v[E::NP][32];
         if (cnt == TILE) load_tile_vec<E>(kin, vin, base, lane, v);
         else load_tile_guarded<E>(kin, vin, base, cnt, lane, v);    // missing elements: the maximum element

@@ -106,11 +106,12 @@ __device__ __forceinline__ SelElem sel_load(const void *kin, const uint32_t *vin
 
 constexpr int PART4_THREADS = 128;
 template <class E>
-__global__ void __launch_bounds__(PART4_THREADS)
+__global__ void __launch_bounds__(PART4_THREADS, 1)
 partition4_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint4 *__restrict__ splits,
                   const unsigned long long n, const unsigned long long L, const unsigned long long num_bounds,
                   const unsigned long long share)
 {
+    pdl_entry();
     const unsigned long long s = static_cast<unsigned long long>(blockIdx.x) * PART4_THREADS + threadIdx.x;
     if (s >= num_bounds) return;
     const unsigned long long out0 = s * share;
@@ -325,6 +326,7 @@ merge4_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ v
                    uint32_t *__restrict__ vout, const uint4 *__restrict__ splits, const unsigned long long n,
                    const unsigned long long L, const unsigned long long num_shares)
 {
+    pdl_entry();
     using C = Cfg4<E>;
     constexpr int KB = C::KB;
     extern __shared__ __align__(128) unsigned char smem_raw[];

@@ -63,6 +63,10 @@ struct Cfg {
     static constexpr size_t total = bar_off + 2 * NSTAGE * 8;
     // 227 KiB of shared memory per SM, 1 KiB per CTA reserved by the system
     static constexpr int ctas_per_sm = (2 * (total + 1024) <= 227 * 1024) ? 2 : 1;
+    // registers per thread that keep ctas_per_sm CTAs of (NW + 1) warps resident (64 K registers per SM, allocation
+    // unit 8): stated to ptxas as the cap itself (__maxnreg__), because with __launch_bounds__ alone it settles on
+    // fewer registers than the SM offers and spills a word for the three-plane element type
+    static constexpr int max_regs = (65536 / ((NW + 1) * 32 * ctas_per_sm)) / 8 * 8;
 };
 
 // ------------------------------------------------------------------ PTX wrappers (mbarrier, TMA)
@@ -170,6 +174,7 @@ __global__ void __launch_bounds__(PART_THREADS)
 partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
                        const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)
 {
+    pdl_entry();
     const int j = threadIdx.x % G;                       // lane inside the group
     const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     const unsigned long long s = (static_cast<unsigned long long>(blockIdx.x) * PART_THREADS + threadIdx.x) / G;
@@ -343,6 +348,7 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
                   uint32_t *__restrict__ vout, const uint32_t *__restrict__ splits, const unsigned long long n,
                   const unsigned long long L, const unsigned long long num_shares)
 {
+    pdl_entry();
     using C = Cfg<E>;
     constexpr int KB = C::KB;
     extern __shared__ __align__(128) unsigned char smem_raw[];

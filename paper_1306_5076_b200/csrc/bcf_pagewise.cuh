@@ -61,6 +61,7 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32)
 pagewise_merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
                       void *__restrict__ kout, uint32_t *__restrict__ vout, const size_t n, const size_t run_len)
 {
+    pdl_entry();
     constexpr int NP = E::NP;
     constexpr int H = TILE / 2;
     extern __shared__ __align__(16) uint32_t smem[];
@@ -70,12 +71,14 @@ pagewise_merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__
     const size_t pair = static_cast<size_t>(blockIdx.x) * WARPS_PER_CTA + warp;
     const size_t a0 = pair * 2 * run_len;
     if (a0 >= n) return;
-    size_t len[2], start[2], ic[2] = {0, 0};
-    len[0] = min(run_len, n - a0);
-    start[0] = a0;
-    start[1] = a0 + len[0];
-    len[1] = min(run_len, n - start[1]);
-    const size_t total = len[0] + len[1];
+    // two scalars and a select per stream quantity: an array indexed by the runtime stream number `e`
+    // would live in local memory
+    const size_t len0 = min(run_len, n - a0);
+    const size_t start0 = a0;
+    const size_t start1 = a0 + len0;
+    const size_t len1 = min(run_len, n - start1);
+    size_t ic0 = 0, ic1 = 0;
+    const size_t total = len0 + len1;
     size_t oc = 0;
     int e;
 
@@ -86,24 +89,24 @@ pagewise_merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         const size_t q = 32 * k + lane;
-        if (q < len[0]) load_elem<E>(kin, vin, start[0] + q, v, k);
+        if (q < len0) load_elem<E>(kin, vin, start0 + q, v, k);
         else set_sentinel<E>(v, k);
     }
 #pragma unroll
     for (int k = 16; k < 32; ++k) {
         const size_t q = TILE - 1 - (32 * k + lane);
-        if (q < len[1]) load_elem<E>(kin, vin, start[1] + q, v, k);
+        if (q < len1) load_elem<E>(kin, vin, start1 + q, v, k);
         else set_sentinel<E>(v, k);
     }
-    ic[0] = min(static_cast<size_t>(H), len[0]);
-    ic[1] = min(static_cast<size_t>(H), len[1]);
+    ic0 = min(static_cast<size_t>(H), len0);
+    ic1 = min(static_cast<size_t>(H), len1);
     // L466-468: the stream whose page will be exhausted first (e = 0 restored, reading A9).
     {
         uint32_t s0[NP], s1[NP];
 #pragma unroll
         for (int p = 0; p < NP; ++p) s0[p] = s1[p] = SENTINEL;
-        if (len[0] >= static_cast<size_t>(H)) load_scalar<E>(kin, vin, start[0] + H - 1, s0);
-        if (len[1] >= static_cast<size_t>(H)) load_scalar<E>(kin, vin, start[1] + H - 1, s1);
+        if (len0 >= static_cast<size_t>(H)) load_scalar<E>(kin, vin, start0 + H - 1, s0);
+        if (len1 >= static_cast<size_t>(H)) load_scalar<E>(kin, vin, start1 + H - 1, s1);
         e = planes_lt<NP>(s1, s0) ? 1 : 0;           // S[M/2-1] <= S[M-1]  ->  e = 0
     }
 
@@ -128,21 +131,22 @@ pagewise_merge_kernel(const void *__restrict__ kin, const uint32_t *__restrict__
         oc += H;
 
         // L475: WHILE (ic[0] < n) OR (ic[1] < n)
-        more = (ic[0] < len[0]) || (ic[1] < len[1]);
+        more = (ic0 < len0) || (ic1 < len1);
         if (!more) break;
-        if (ic[e] >= len[e]) e = 1 - e;              // L478
-        const size_t ls = min(static_cast<size_t>(H), len[e] - ic[e]);   // L420
+        if ((e ? ic1 : ic0) >= (e ? len1 : len0)) e = 1 - e;              // L478
+        const size_t len_e = e ? len1 : len0, ic_e = e ? ic1 : ic0, start_e = e ? start1 : start0;
+        const size_t ls = min(static_cast<size_t>(H), len_e - ic_e);   // L420
         // L479: S[0..M/2) = next page of stream e (padded with infinity)
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
             const size_t q = 32 * k + lane;
-            if (q < ls) load_elem<E>(kin, vin, start[e] + ic[e] + q, v, k);
+            if (q < ls) load_elem<E>(kin, vin, start_e + ic_e + q, v, k);
             else set_sentinel<E>(v, k);
         }
 #pragma unroll
         for (int p = 0; p < NP; ++p) last_new[p] = SENTINEL;
-        if (ls == static_cast<size_t>(H)) load_scalar<E>(kin, vin, start[e] + ic[e] + H - 1, last_new);
-        ic[e] += ls;                                 // L480
+        if (ls == static_cast<size_t>(H)) load_scalar<E>(kin, vin, start_e + ic_e + H - 1, last_new);
+        if (e) ic1 += ls; else ic0 += ls;            // L480
         if (planes_lt<NP>(top, last_new)) e = 1 - e; // L482: IF S[M/2-1] > S[M-1]
         // the kept upper half, reversed behind the new page: position 32k + lane, k >= 16, holds
         // sorted element (47 - k, 31 - lane); one shared-memory line per k -> conflict-free.

@@ -214,9 +214,7 @@ def test_argument_errors_are_reported_before_any_device_work():
     INVALID, MISALIGNED, TOO_SMALL = 1, 2, 3
     buf = np.zeros(1 << 16, dtype=np.uint8)
     p = (buf.ctypes.data + 255) & ~255
-    assert L.bcf_set_base_case(7) == INVALID and L.bcf_set_rounds_per_pass(3) == INVALID
-    assert L.bcf_set_base_case(3) == 0 and L.bcf_get_base_case() == 3
-    assert L.bcf_set_rounds_per_pass(1) == 0 and L.bcf_get_rounds_per_pass() == 1
+    assert L.bcf_options_init(None) == INVALID
     assert L.bcf_sort_long_tiles(p, None, 1, 3, 0, 0, None) == INVALID                 # h must be 2, 4 or 8
     assert L.bcf_sort_long_tiles(p + 4, None, 1, 2, 0, 0, None) == MISALIGNED
     assert L.bcf_sort_tiles_mergesort(None, None, 1, 0, 0, None) == INVALID
@@ -238,11 +236,26 @@ def test_argument_errors_are_reported_before_any_device_work():
     assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 4, 0, p, p + 32768, ws, None) == INVALID          # out aliases values
     assert L.bcf_colored_prefix_sums(p, p + 8192, 1000, 4, 0, p + 16384, p + 32768, 0, None) == TOO_SMALL
     # pass structure of the merging phase (host only)
-    assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0) == 18 and L.bcf_merge_pass_count(1 << 28, 8192, 0, 0) == 15
-    assert L.bcf_set_rounds_per_pass(2) == 0
-    try:
-        assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0) == 9
-        assert L.bcf_merge_pass_count(1 << 27, 1024, 0, 0) == 9     # 17 rounds: one two-way pass + 8 four-run passes
-        assert L.bcf_merge_pass_count(1 << 26, 1024, 1, 1) == 16    # (u64,u32): the four-run stage buffers do not fit
-    finally:
-        L.bcf_set_rounds_per_pass(1)
+    one, two = ctypes.byref(bcf.options(rounds_per_pass=1)), ctypes.byref(bcf.options(rounds_per_pass=2))
+    assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0, one) == 18 and L.bcf_merge_pass_count(1 << 28, 8192, 0, 0, one) == 15
+    assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0, two) == 9
+    assert L.bcf_merge_pass_count(1 << 27, 1024, 0, 0, two) == 9     # 17 rounds: one two-way pass + 8 four-run passes
+    assert L.bcf_merge_pass_count(1 << 26, 1024, 1, 1, two) == 16    # (u64,u32): the four-run stage buffers do not fit
+    # the two option sets do not interact: no process-wide state is left behind by either call
+    assert L.bcf_merge_pass_count(1 << 28, 1024, 0, 0, one) == 18 and L.bcf_merge_pass_count(1 << 28, 1024, 0, 0, two) == 9
+    # bcf_options validation (host side, before any device work)
+    bad = bcf.options()
+    bad.base_case = 9
+    assert L.bcf_sort_ex(p, None, 4096, 0, 0, p + 32768, 1 << 15, None, ctypes.byref(bad)) == INVALID
+    bad = bcf.options()
+    bad.struct_size = 8
+    assert L.bcf_merge_pass_count(1 << 20, 1024, 0, 0, ctypes.byref(bad)) == 0
+    # BCFMergesort with buckets: P >= 2, t >= 1, workspace
+    assert L.bcf_sort_buckets_workspace_bytes(1 << 20, 8, 1, 0, 0) == 0 and L.bcf_sort_buckets_workspace_bytes(1 << 20, 0, 8, 0, 0) == 0
+    need = L.bcf_sort_buckets_workspace_bytes(1 << 14, 4, 4, 1, 0)
+    assert need >= 2 * 4 * (1 << 14)
+    assert L.bcf_sort_buckets(p, 1 << 14, 0, 4, 1, 0, None, p, need, None, None) == INVALID
+    assert L.bcf_sort_buckets(p, 1 << 14, 0, 4, 4, 0, None, p + (1 << 20), 64, None, None) == TOO_SMALL
+    assert L.bcf_sort_buckets(p, 0, 0, 4, 4, 0, None, None, 0, None, None) == 0
+    assert L.bcf_merge_pieces_workspace_bytes(1 << 14, 4, 1, 0) > 0 and L.bcf_merge_pieces_workspace_bytes(0, 4, 4, 0) == 0
+    assert L.bcf_merge_pieces(p, p, 100, p, 4, 4, 0, 0, p, 1 << 14, None) == INVALID            # in/out aliasing

@@ -21,22 +21,18 @@ def bcf():
 
 
 @pytest.fixture(params=[1, 2], ids=["1round", "2rounds"])
-def rpp(request, bcf):
-    """Both pass structures of the merging phase: one round per pass (Lemma 2) and two
-    rounds per pass (four-run kernel); the result must be the same unique sorted output."""
-    before = bcf.get_rounds_per_pass()
-    bcf.set_rounds_per_pass(request.param)
-    yield request.param
-    bcf.set_rounds_per_pass(before)
+def rpp(request):
+    """Both pass structures of the merging phase, passed per call in bcf_options: one round per pass
+    (Lemma 2) and two rounds per pass (four-run kernel); the result must be the same unique
+    sorted output."""
+    return request.param
 
 
 @pytest.fixture(params=[0, 1, 2], ids=["shearsort", "tilemergesort", "longtiles"])
-def base(request, bcf):
-    """Both base cases of bcf_sort: the paper's tile ShearSort and the tile mergesort network."""
-    before = bcf.get_base_case()
-    bcf.set_base_case(request.param)
-    yield request.param
-    bcf.set_base_case(before)
+def base(request):
+    """The base cases of bcf_sort (bcf_options.base_case): the paper's tile ShearSort, the tile mergesort
+    network, long tiles."""
+    return request.param
 
 
 def dev(a):
@@ -231,7 +227,7 @@ def test_merge_runs_matches_oracle(bcf, kind, n, run_len, rpp):
     else:
         keys, vals = workloads.sorted_runs(keys, run_len, vals)
     dk, dv = dev(keys), dev(vals)
-    out = bcf.merge_runs(dk, run_len, dv)
+    out = bcf.merge_runs(dk, run_len, dv, opts={"rounds_per_pass": rpp})
     want = oracle.merge_runs(keys, run_len, vals)
     if vals is None:
         assert np.array_equal(host(out, keys), want)
@@ -243,7 +239,7 @@ def test_merge_runs_matches_oracle(bcf, kind, n, run_len, rpp):
 @pytest.mark.parametrize("k", [2, 64, 1024])
 def test_merge_runs_config5b_shape(bcf, k, rpp):
     keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=1 << 18)
-    out = bcf.merge_runs(dev(keys), run_len)
+    out = bcf.merge_runs(dev(keys), run_len, opts={"rounds_per_pass": rpp})
     assert np.array_equal(host(out, keys), oracle.merge_runs(keys, run_len))
 
 
@@ -285,27 +281,41 @@ def test_merge_runs_pagewise_matches_oracle(bcf, kind, n, run_len):
 def test_sort_matches_oracle(bcf, kind, n, rpp, base):
     keys, vals = make(kind, n, seed=n, dup=(n % 3 == 0))
     dk, dv = dev(keys), dev(vals)
-    bcf.sort(dk, dv)
+    bcf.sort(dk, dv, opts={"rounds_per_pass": rpp, "base_case": base})
     want = oracle.sort_full(keys, vals)
     assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+@pytest.mark.parametrize("launch_mode", [1, 2], ids=["plain", "pdl"])
+@pytest.mark.parametrize("n", [1 << 17, 300001])
+def test_sort_launch_modes(bcf, n, rpp, launch_mode):
+    """Ordinary and programmatic dependent launches (bcf_options.launch_mode) give the same result."""
+    for kind in ("u32", "u64u32"):
+        keys, vals = make(kind, n, seed=n + launch_mode)
+        dk, dv = dev(keys), dev(vals)
+        for _ in range(3):                                   # back-to-back calls on one stream
+            dk.copy_(dev(keys))
+            bcf.sort(dk, dv if vals is None else dv.copy_(dev(vals)), opts={"rounds_per_pass": rpp, "launch_mode": launch_mode})
+        want = oracle.sort_full(keys, vals)
+        assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
 
 
 @pytest.mark.parametrize("dist", workloads.CFG4_VARIANTS)
 def test_sort_config4_distributions(bcf, dist, rpp, base):
     keys = workloads.cfg4_sort_u32(dist, n=(1 << 18) + 1000)
     d = dev(keys)
-    bcf.sort(d)
+    bcf.sort(d, opts={"rounds_per_pass": rpp, "base_case": base})
     assert np.array_equal(host(d, keys), oracle.sort_full(keys))
 
 
 def test_sort_config3_and_5a_shapes(bcf, rpp):
     keys = workloads.cfg3_sort_u32(n=1 << 19)
     d = dev(keys)
-    bcf.sort(d)
+    bcf.sort(d, opts={"rounds_per_pass": rpp})
     assert np.array_equal(host(d, keys), oracle.sort_full(keys))
     k, v = workloads.cfg5a_sort_u64_u32(n=(1 << 18) + 3)
     dk, dv = dev(k), dev(v)
-    bcf.sort(dk, dv)
+    bcf.sort(dk, dv, opts={"rounds_per_pass": rpp})
     wk, wv = oracle.sort_full(k, v)
     assert np.array_equal(host(dk, k), wk) and np.array_equal(host(dv, v), wv)
 
@@ -347,13 +357,82 @@ def test_error_codes(bcf):
         bcf.sort(k.cpu())                                         # no CPU path
 
 
-def test_kernels_use_no_local_memory(bcf):
-    for cls in ("tile_sort", "partition", "merge", 4):   # 4 = BCF_KERNEL_TILE_MERGESORT
+# Local memory (stack) bytes per thread the build is allowed to have, by (kernel, key type, value type).
+# makes "the data is not transferred to local memory" part of the method: every kernel must show 0 unless it is
+# listed here with the exact byte count (DESIGN.md section 4 names each entry and why it is not a data spill).
+LOCAL_BYTES_ALLOWED = {
+    # one scratch-plane address computed before the share loop, stored once and re-read once per share (STL/LDL
+    # of R2 in SASS); ptxas settles on 168 registers although the launch bound allows 224.  Not element data.
+    ("merge_pipe", 1, 1): 8,
+}
+
+
+def test_every_launched_kernel_uses_no_local_memory(bcf):
+    """All 14 kernels x 4 element types (those that exist): cudaFuncGetAttributes().localSizeBytes == 0."""
+    seen = 0
+    for kid in bcf.KERNEL_IDS:
         for kt in (0, 1):
             for vt in (0, 1):
-                info = bcf.kernel_info(cls, kt, vt)
-                assert info["local_bytes_per_thread"] == 0, (cls, kt, vt, info)
-                assert info["ctas_per_sm"] >= 1
+                try:
+                    info = bcf.kernel_info(kid, kt, vt)
+                except bcf.BcfError as e:
+                    assert e.name == "BCF_ERR_INVALID_ARG"
+                    assert (kid == "merge4_pipe" and (kt, vt) == (1, 1)) or (kid == "merge_pieces" and vt == 1), (kid, kt, vt)
+                    continue
+                seen += 1
+                assert info["local_bytes_per_thread"] == LOCAL_BYTES_ALLOWED.get((kid, kt, vt), 0), (kid, kt, vt, info)
+                assert info["ctas_per_sm"] >= 1, (kid, kt, vt, info)
+    assert seen == 14 * 4 - 1 - 2
+
+
+def test_options_are_per_call_and_validated(bcf):
+    """No process-wide settings: two option sets in alternation give their own pass structure every time."""
+    keys, _ = make("u32", 1 << 17, seed=9)
+    want = oracle.sort_full(keys)
+    for i in range(4):
+        o = {"rounds_per_pass": 1 + i % 2, "base_case": i % 3}
+        bcf.launch_counts()
+        d = dev(keys)
+        bcf.sort(d, opts=o)
+        torch.cuda.synchronize()
+        launches = bcf.launch_counts()
+        run = 8192 if o["base_case"] == 2 else 1024
+        assert launches["merge"] == bcf.merge_pass_count(keys.size, run, "uint32", opts={"rounds_per_pass": o["rounds_per_pass"]})
+        assert np.array_equal(host(d, keys), want)
+    bad = bcf.options()
+    bad.rounds_per_pass = 7
+    with pytest.raises(bcf.BcfError) as e:
+        bcf.sort(dev(keys), opts=bad)
+    assert e.value.name == "BCF_ERR_INVALID_ARG"
+    bad = bcf.options()
+    bad.struct_size = 4
+    with pytest.raises(bcf.BcfError):
+        bcf.sort(dev(keys), opts=bad)
+
+
+def test_a_failed_launch_is_reported_once_and_does_not_stick(bcf):
+    """include/bcf.h ERRORS: a pending CUDA error of another library call is cleared on entry; the next call works."""
+    k = torch.zeros(4096, dtype=torch.int32, device="cuda")
+    try:
+        torch.empty(1, device="cuda").new_empty((1 << 62,))       # a failing CUDA call (out of memory) in this thread
+    except Exception:
+        pass
+    bcf.sort(k)                                                   # must not return BCF_ERR_CUDA because of it
+    torch.cuda.synchronize()
+
+
+def test_second_device_in_one_process(bcf):
+    """Per-device caches (kernel attributes, SM count) are keyed by device id: sort on cuda:1 after cuda:0."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs")
+    keys, vals = make("u64u32", 70000, seed=4)
+    want = oracle.sort_full(keys, vals)
+    for d in (0, 1, 0):
+        with torch.cuda.device(d):
+            dk = torch.from_numpy(keys.view(np.int64)).to(f"cuda:{d}")
+            dv = torch.from_numpy(vals.view(np.int32)).to(f"cuda:{d}")
+            bcf.sort(dk, dv)
+            assert np.array_equal(dk.cpu().numpy().view(np.uint64), want[0])
 
 
 # ---------------------------------------------------------------- bcf_find_buckets (SURVEY 8f item 2)
@@ -399,3 +478,77 @@ def test_colored_prefix_sums_match_oracle(bcf, layout, n, d):
         cols[100:1500] = d - 1                      # a long single-colour stretch
     out = bcf.colored_prefix_sums(dev(vals), torch.from_numpy(cols).cuda(), d, layout=layout)
     assert np.array_equal(host(out, vals), oracle.colored_prefix_sums(vals, cols, d))
+
+
+# ---------------------------------------------------------------- bcf_sort_buckets / bcf_merge_pieces
+
+
+@pytest.mark.parametrize("kind", ["u32", "u64"])
+@pytest.mark.parametrize("pb", [False, True], ids=["plain", "pivot_buckets"])
+@pytest.mark.parametrize("n,P,t,data", [
+    (64 * 1024, 8, 8, "uniform"), (64 * 1024 + 777, 8, 8, "dup"), (300001, 16, 16, "uniform"), (1 << 18, 16, 4, "zero_one"),
+    (1 << 18, 128, 128, "uniform"), (5000, 4, 4, "dup"), (1024, 4, 4, "uniform"), (200000, 3, 5, "dup256"), (1 << 20, 32, 32, "zero_one"),
+])
+def test_sort_buckets_matches_oracle(bcf, kind, pb, n, P, t, data, base):
+    """BCFMergesort with FIND-BUCKETS and the bucket-local final merge phase (BCFMergesortPB with pivot buckets):
+    the unique sorted output, element by element, against oracle.sort_full_buckets (PAPER.md 3.2, App. B)."""
+    rng = np.random.default_rng(n + P + t)
+    dt = np.uint32 if kind == "u32" else np.uint64
+    if data == "uniform":
+        keys = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(dt)
+        if kind == "u64":
+            keys = (keys << np.uint64(32)) | rng.integers(0, 1 << 32, size=n, dtype=np.uint64)
+    elif data == "dup":
+        keys = rng.integers(0, 16, size=n).astype(dt)
+    elif data == "dup256":
+        keys = rng.integers(0, 1 << 32, size=256, dtype=np.uint64).astype(dt)[rng.integers(0, 256, size=n)]
+    else:
+        keys = rng.integers(0, 2, size=n).astype(dt)
+    keys[n // 3] = np.iinfo(dt).max                              # the padding value is a legal key (A10)
+    d = dev(keys)
+    bcf.sort_buckets(d, P, t=t, pivot_buckets=pb, opts={"base_case": base})
+    want = oracle.sort_full_buckets(keys, P, t=t, pivot_buckets=pb) if n <= (1 << 18) else np.sort(keys)
+    assert np.array_equal(host(d, keys), want)
+
+
+def test_sort_buckets_bucket_starts_match_oracle_and_lemma_1(bcf):
+    """The distribution inside bcf_sort_buckets is the oracle's (same runs, same pivots): bucket starts equal,
+    and with all keys distinct no bucket exceeds Lemma 1's bound s ceil(N/(s t)) + ceil(s t/P) ceil(N/(s t))."""
+    n, P, t = 1 << 18, 16, 16
+    keys = np.random.default_rng(1).permutation(1 << 20)[:n].astype(np.uint32)
+    d = dev(keys)
+    _, starts = bcf.sort_buckets(d, P, t=t, opts={"base_case": 1}, return_bucket_starts=True)
+    out, info = oracle.sort_full_buckets(keys, P, t=t, return_info=True)
+    assert np.array_equal(host(d, keys), out)
+    got = starts.cpu().numpy().astype(np.int64)
+    assert np.array_equal(np.diff(got), np.array(info["bucket_sizes"]))
+    s = info["s"]
+    per = -(-n // (s * t))
+    assert np.diff(got).max() <= s * per + (-(-(s * t) // P)) * per
+
+
+@pytest.mark.parametrize("kind", ["u32", "u64"])
+@pytest.mark.parametrize("groups,s,copy_odd", [(1, 2, False), (5, 3, False), (7, 8, True), (3, 1, False), (16, 16, False), (9, 5, True)])
+def test_merge_pieces_matches_oracle(bcf, kind, groups, s, copy_odd):
+    """The final merge phase alone: ragged, empty and page-spanning pieces; pivot buckets (odd groups) are copied."""
+    rng = np.random.default_rng(groups * 100 + s)
+    dt = np.uint32 if kind == "u32" else np.uint64
+    lens = rng.choice([0, 1, 5, 31, 700, 1024, 1500, 3000], size=groups * s)
+    offs = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    n = int(offs[-1])
+    if n == 0:
+        pytest.skip("empty draw")
+    keys = np.empty(n, dtype=dt)
+    want = np.empty(n, dtype=dt)
+    for g in range(groups):
+        lo, hi = offs[g * s], offs[(g + 1) * s]
+        if copy_odd and g % 2 == 1:
+            keys[lo:hi] = dt(rng.integers(0, 1000))              # a pivot bucket: copies of one key
+        else:
+            for r in range(s):
+                a, b = offs[g * s + r], offs[g * s + r + 1]
+                keys[a:b] = np.sort(rng.integers(0, 50 if g % 3 == 0 else 1 << 31, size=b - a).astype(dt))
+        merged, _ = oracle.merge_pieces([keys[offs[g * s + r]:offs[g * s + r + 1]] for r in range(s)])
+        want[lo:hi] = merged
+    out = bcf.merge_pieces(dev(keys), torch.from_numpy(offs.astype(np.int32)).cuda(), groups, s, copy_odd_groups=copy_odd)
+    assert np.array_equal(host(out, keys), want)
