@@ -356,6 +356,24 @@ bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in,
                                    void *d_vals_out, size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
                                    void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
 
+/* ------------------------------------------------------------------ debug: conflict isolation --- */
+
+/*
+ * The bank-conflict isolation experiment (csrc/bcf_tu_isolate.cu; profiles/r2_conflict_isolation.md).  DEBUG entry
+ * points: nothing in the library calls them.  They run the same shared-memory instruction streams as
+ * merge_pipe_kernel and tile_mergesort_kernel (uint32 keys) in three phases separated by CTA barriers --
+ * global -> chip, every LDS / STS of the work item, registers -> global -- so that ncu's
+ * l1tex__data_bank_conflicts_pipe_lsu_mem_shared_op_{ld,st} can be read with (exclusive = 0, several CTAs per SM)
+ * and without (exclusive = 1, one CTA per SM) other global-memory traffic on the SM during the LDS / STS phase.
+ *   bcf_debug_merge_round_isolated : ONE merge round of runs of run_len = 8192 * 2^k; n a multiple of
+ *       2 run_len; out of place; d_workspace >= (n / BCF_SHARE + 1) * 4 bytes (split points, production kernel).
+ *   bcf_debug_sort_tiles_isolated  : bcf_sort_tiles_mergesort of whole tiles, in place.
+ * Results are those of bcf_merge_runs / bcf_sort_tiles (parity-tested).
+ */
+bcf_status bcf_debug_merge_round_isolated(const void *d_keys_in, void *d_keys_out, size_t n, size_t run_len, int exclusive,
+                                          void *d_workspace, size_t workspace_bytes, bcf_stream_t stream);
+bcf_status bcf_debug_sort_tiles_isolated(void *d_keys, size_t num_tiles, int exclusive, bcf_stream_t stream);
+
 /* ------------------------------------------------------------------ measurement hooks ------ */
 
 typedef enum {

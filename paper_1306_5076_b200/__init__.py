@@ -27,6 +27,8 @@ from .binding import (  # noqa: F401
     merge_partition4,
     merge_pass_count,
     merge_pieces,
+    debug_merge_round_isolated,
+    debug_sort_tiles_isolated,
     sort_buckets,
     options,
     Options,

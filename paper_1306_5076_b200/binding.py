@@ -109,6 +109,8 @@ def lib():
     L.bcf_merge_pieces_workspace_bytes.restype = sz
     L.bcf_merge_pieces_workspace_bytes.argtypes = [sz, sz, sz, ci]
     L.bcf_merge_pieces.argtypes = [vp, vp, sz, vp, sz, sz, ci, ci, vp, sz, vp]
+    L.bcf_debug_merge_round_isolated.argtypes = [vp, vp, sz, sz, ci, vp, sz, vp]
+    L.bcf_debug_sort_tiles_isolated.argtypes = [vp, sz, ci, vp]
     L.bcf_profile_enable.argtypes = [ci]
     L.bcf_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u64)]
     L.bcf_launch_counts.argtypes = [ctypes.POINTER(u64)]
@@ -382,6 +384,29 @@ def sort_host(keys, vals=None, scratch=None, device="cuda", stream=None, opts=No
     _check(lib().bcf_sort_host_ex(keys.data_ptr(), None if vals is None else vals.data_ptr(), n, kt, vt,
                                   scratch.data_ptr(), scratch.numel(), _stream(stream), _opt(opts)), "bcf_sort_host_ex")
     return keys if vals is None else (keys, vals)
+
+
+def debug_merge_round_isolated(keys, run_len, exclusive=True, out_keys=None, stream=None):
+    """bcf_debug_merge_round_isolated: one merge round of uint32 runs with the phase-separated kernel (experiment)."""
+    torch = _torch()
+    n = keys.numel()
+    if out_keys is None:
+        out_keys = torch.empty_like(keys)
+    ws = torch.empty((n // SHARE + 1) * 4 + 16, dtype=torch.uint8, device=keys.device)
+    _check(lib().bcf_debug_merge_round_isolated(_dev(keys, "keys"), _dev(out_keys, "out_keys"), n, int(run_len),
+                                                int(bool(exclusive)), ws.data_ptr(), ws.numel(), _stream(stream)),
+           "bcf_debug_merge_round_isolated")
+    return out_keys
+
+
+def debug_sort_tiles_isolated(keys, exclusive=True, stream=None):
+    """bcf_debug_sort_tiles_isolated: tile mergesort of uint32 tiles with the phase-separated kernel (experiment)."""
+    n = keys.numel()
+    if n % TILE:
+        raise ValueError("whole tiles only")
+    _check(lib().bcf_debug_sort_tiles_isolated(_dev(keys, "keys"), n // TILE, int(bool(exclusive)), _stream(stream)),
+           "bcf_debug_sort_tiles_isolated")
+    return keys
 
 
 def profile_enable(on=True):

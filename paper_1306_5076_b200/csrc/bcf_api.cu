@@ -875,6 +875,44 @@ bcf_status bcf_sort_host(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, bcf
     return bcf_sort_host_ex(h_keys, h_vals, n, kt, vt, d_scratch, scratch_bytes, stream, nullptr);
 }
 
+// ------------------------------------------------------------------ bank-conflict isolation experiment (debug)
+
+bcf_status bcf_debug_merge_round_isolated(const void *d_keys_in, void *d_keys_out, size_t n, size_t run_len, int exclusive,
+                                          void *d_workspace, size_t workspace_bytes, bcf_stream_t stream)
+{
+    if (n == 0) return BCF_OK;
+    if (n >= (size_t(1) << 32) || run_len < BCF_SHARE || (run_len & (run_len - 1)) || n % (2 * run_len)) return BCF_ERR_INVALID_ARG;
+    if (!d_keys_in || !d_keys_out || !d_workspace) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
+    if (overlap(d_keys_in, n * 4, d_keys_out, n * 4)) return BCF_ERR_INVALID_ARG;
+    if (workspace_bytes < (n / BCF_SHARE + 1) * 4) return BCF_ERR_WORKSPACE_TOO_SMALL;
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    bcf_status st = current_device(&c.dev);
+    if (st != BCF_OK) return st;
+    ProfileGroup profile_group(stream);
+    uint32_t *splits = static_cast<uint32_t *>(d_workspace);
+    st = launch_partition_share<E_U32>(c, d_keys_in, nullptr, splits, n, run_len);
+    if (st != BCF_OK) return st;
+    return launch_isolated_merge_round(c, static_cast<const uint32_t *>(d_keys_in), static_cast<uint32_t *>(d_keys_out), splits, n,
+                                       run_len, exclusive);
+}
+
+bcf_status bcf_debug_sort_tiles_isolated(void *d_keys, size_t num_tiles, int exclusive, bcf_stream_t stream)
+{
+    if (num_tiles == 0) return BCF_OK;
+    if (num_tiles >= (size_t(1) << 22) || !d_keys) return BCF_ERR_INVALID_ARG;
+    if (!aligned16(d_keys)) return BCF_ERR_MISALIGNED;
+    Call c;
+    c.s = stream;
+    resolve_options(nullptr, &c.opt);
+    const bcf_status st = current_device(&c.dev);
+    if (st != BCF_OK) return st;
+    ProfileGroup profile_group(stream);
+    return launch_isolated_tile_mergesort(c, static_cast<uint32_t *>(d_keys), num_tiles, exclusive);
+}
+
 // ------------------------------------------------------------------ measurement hooks
 
 bcf_status bcf_profile_enable(int on)

@@ -176,6 +176,8 @@ template <class E>
 bool kernel_desc_merge(int id, KernelDesc *k);
 // bcf_tu_pipe.cu
 template <class E>
+bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len);
+template <class E>
 bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits,
                              size_t n, size_t run_len);
 template <class E>
@@ -205,6 +207,11 @@ size_t colored_scan_workspace_bytes(size_t n);
 int colored_scan_max_colors();
 bcf_status launch_colored_scan(const Call &c, const uint32_t *values, const uint8_t *colors, size_t n, int num_colors, bool cf,
                                uint32_t *partial, uint32_t *out);
+
+// bcf_tu_isolate.cu: the bank-conflict isolation experiment (debug entry points of include/bcf.h)
+bcf_status launch_isolated_merge_round(const Call &c, const uint32_t *kin, uint32_t *kout, const uint32_t *splits, size_t n,
+                                       size_t run_len, int exclusive);
+bcf_status launch_isolated_tile_mergesort(const Call &c, uint32_t *keys, size_t num_tiles, int exclusive);
 
 // the four element types every templated launcher is instantiated for
 using E_U32 = Elem<1, false>;

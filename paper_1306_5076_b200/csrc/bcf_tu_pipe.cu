@@ -5,6 +5,22 @@
 
 namespace bcf {
 
+// split points of the share boundaries of one round (only rounds with 2 L > SH need them)
+template <class E>
+bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len)
+{
+    const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
+    const unsigned long long ull_n = n, ull_l = run_len;
+    LaunchTimer t(BCF_KERNEL_PARTITION, c.s);
+    // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
+    if (shares + 1 <= c.opt.warp_search_max) {
+        const unsigned blocks = static_cast<unsigned>(((shares + 1) * 32 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
+        return launch(c, pipe::partition_share_kernel<E, 32>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
+    }
+    const unsigned blocks = static_cast<unsigned>((shares + 1 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
+    return launch(c, pipe::partition_share_kernel<E, 1>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
+}
+
 template <class E>
 bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits,
                              size_t n, size_t run_len)
@@ -14,24 +30,16 @@ bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin
     if (shares == 0) return BCF_OK;
     bcf_status st = ensure_dyn_smem<pipe::merge_pipe_kernel<E>>(c.dev, C::total);
     if (st != BCF_OK) return st;
-    const unsigned long long ull_n = n, ull_l = run_len;
     if (2 * run_len > (size_t)pipe::SH) {
-        LaunchTimer t(BCF_KERNEL_PARTITION, c.s);
-        // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
-        if (shares + 1 <= c.opt.warp_search_max) {
-            const unsigned blocks = static_cast<unsigned>(((shares + 1) * 32 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-            st = launch(c, pipe::partition_share_kernel<E, 32>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
-        } else {
-            const unsigned blocks = static_cast<unsigned>((shares + 1 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-            st = launch(c, pipe::partition_share_kernel<E, 1>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
-        }
+        st = launch_partition_share<E>(c, kin, vin, splits, n, run_len);
         if (st != BCF_OK) return st;
     }
     LaunchTimer t(BCF_KERNEL_MERGE, c.s);
     const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * c.dev.num_sms;
     const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
     return launch(c, pipe::merge_pipe_kernel<E>, blocks, pipe::THREADS, C::total, kin, vin, kout, vout,
-                  static_cast<const uint32_t *>(splits), ull_n, ull_l, shares);
+                  static_cast<const uint32_t *>(splits), static_cast<unsigned long long>(n),
+                  static_cast<unsigned long long>(run_len), shares);
 }
 
 template <class E>
@@ -45,12 +53,16 @@ bool kernel_desc_pipe(int id, KernelDesc *k)
     return false;
 }
 
+template bcf_status launch_partition_share<E_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U32>(int, KernelDesc *);
+template bcf_status launch_partition_share<E_U32_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U32_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U32_U32>(int, KernelDesc *);
+template bcf_status launch_partition_share<E_U64>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U64>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U64>(int, KernelDesc *);
+template bcf_status launch_partition_share<E_U64_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U64_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U64_U32>(int, KernelDesc *);
 

@@ -552,3 +552,35 @@ def test_merge_pieces_matches_oracle(bcf, kind, groups, s, copy_odd):
         want[lo:hi] = merged
     out = bcf.merge_pieces(dev(keys), torch.from_numpy(offs.astype(np.int32)).cuda(), groups, s, copy_odd_groups=copy_odd)
     assert np.array_equal(host(out, keys), want)
+
+
+# ---------------------------------------------------------------- debug: conflict-isolation variants
+
+
+@pytest.mark.parametrize("exclusive", [True, False])
+def test_isolated_experiment_kernels_match_oracle(bcf, exclusive):
+    """The phase-separated kernels of the bank-conflict experiment compute what the production kernels compute."""
+    keys, _ = make("u32", 37 * 1024, seed=5)
+    d = dev(keys)
+    bcf.debug_sort_tiles_isolated(d, exclusive=exclusive)
+    assert np.array_equal(host(d, keys), oracle.shearsort_tiles(keys))
+    n, L = 1 << 17, 1 << 14
+    keys, _ = make("u32", n, seed=6, dup=not exclusive)
+    keys = workloads.sorted_runs(keys, L)
+    out = bcf.debug_merge_round_isolated(dev(keys), L, exclusive=exclusive)
+    assert np.array_equal(host(out, keys), oracle.merge_round(keys, L))
+
+
+def test_sort_is_deterministic_under_repetition(bcf):
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md): a race in the hand-rolled barriers would show
+    as a run-to-run difference.  20 repetitions per option set on sizes that exercise every kernel; all bit-identical
+    and equal to the oracle."""
+    for kind, n in (("u32", (1 << 18) + 4099), ("u64u32", 70001)):
+        keys, vals = make(kind, n, seed=77, dup=True)
+        want = oracle.sort_full(keys, vals)
+        for o in ({"rounds_per_pass": 1, "base_case": 2}, {"rounds_per_pass": 2, "base_case": 2, "launch_mode": 2},
+                  {"rounds_per_pass": 2, "base_case": 1}, {"rounds_per_pass": 1, "base_case": 0, "merge_impl": 1}):
+            for rep in range(20):
+                dk, dv = dev(keys), dev(vals)
+                bcf.sort(dk, dv, opts=o)
+                assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
