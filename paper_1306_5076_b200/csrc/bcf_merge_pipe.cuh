@@ -8,7 +8,8 @@
 // here every CTA takes an equal SHARE of the output of a round instead (north_star: "split-point
 // search so each CTA gets an equal share of output"):
 //
-//   share      = SH = 8 * 1024 consecutive outputs of the round = 8 sub-tiles, one per consumer warp
+//   share      = SH = PAGES * 1024 consecutive outputs of the round (PAGES = 8; 4 for twelve-byte elements), one
+//                page (sub-tile) of 1024 outputs per consumer warp at a time
 //   producer   = one extra warp.  For share s it works out which input the share needs
 //                  - run length 2L <= SH: the share's own input range (whole pairs),
 //                  - otherwise: A[I0, I1) and B[D0 - I0, D1 - I1) from the global split points
@@ -16,7 +17,8 @@
 //                and issues cp.async.bulk (TMA, UBLKCP) copies global -> shared that complete on an
 //                mbarrier.  NSTAGE stage buffers: the copies of share i+1 are in flight while the
 //                consumers work on share i; no load ever occupies a register or an LSU slot.
-//   consumers  = 8 warps.  Each finds the two split points of its own sub-tile INSIDE shared memory
+//   consumers  = NWC warps (8 / 15 / 11 for 4- / 8- / 12-byte elements, Cfg below) that take the pages of the
+//                CTA's shares round robin.  Each finds the two split points of its own sub-tile INSIDE shared memory
 //                with a conflict-free 32-ary search (corank_smem), reads its 1024 elements from the
 //                stage buffer straight into the column layout (word address consecutive across
 //                lanes: conflict-free for any offset), releases the stage, and runs SHEARSORT-MERGE
@@ -34,10 +36,7 @@
 namespace bcf {
 namespace pipe {
 
-constexpr int NW = 8;                    // consumer warps per CTA
-constexpr int SH = NW * TILE;            // outputs per share
-constexpr int NSTAGE = 2;
-constexpr int THREADS = (NW + 1) * 32;
+constexpr int NSTAGE = 2;                // stage buffers of the four-run kernel (bcf_merge4.cuh); this kernel: Cfg<E>::STAGES
 constexpr int REGION_SLACK = 128;        // bytes: room for the 16-byte aligned supersets of two pieces
 
 struct ShareMeta {
@@ -51,22 +50,44 @@ struct ShareMeta {
     int pad;
 };
 
+// Shape of the kernel per element type.  A share is PAGES pages of 1024 outputs; NWC consumer warps take the pages
+// of the CTA's shares round robin (page g of the CTA's page sequence goes to warp g mod NWC), so the number of
+// warps is free of the share size: 4-byte elements keep 8 warps = 8 pages and two CTAs per SM; the wider element
+// types cost 2.5-10 times the ALU work per comparator and run ONE CTA per SM (the stage buffers fill it), where 8
+// warps -- two per SM sub-partition -- left the ALU pipe 40 % idle waiting on fixed-latency dependences
+// (profiles/r2a_merge_kv_full.md); they get as many warps as the register file holds, and twelve-byte elements
+// shares of 4 pages in 3 stage buffers so that the warps' scratch planes still fit.
+#ifndef BCF_PIPE_NWC8
+#define BCF_PIPE_NWC8 15     // consumer warps, 8-byte elements
+#endif
+#ifndef BCF_PIPE_NWC12
+#define BCF_PIPE_NWC12 11    // consumer warps, 12-byte elements
+#endif
 template <class E>
 struct Cfg {
     static constexpr int KB = E::KEY_BYTES;
+    static constexpr int EB = KB + (E::HAS_VAL ? 4 : 0);
+    static constexpr int PAGES = EB >= 12 ? 4 : 8;            // pages per share
+    static constexpr int SH = PAGES * TILE;                    // outputs per share
+    static constexpr int STAGES = EB >= 12 ? 3 : 2;
+    static constexpr int NWC = EB == 4 ? 8 : (EB == 8 ? BCF_PIPE_NWC8 : BCF_PIPE_NWC12);
+    static constexpr int THREADS = (NWC + 1) * 32;
     static constexpr size_t key_region = size_t(SH) * KB + REGION_SLACK;
     static constexpr size_t val_region = E::HAS_VAL ? size_t(SH) * 4 + REGION_SLACK : 0;
     static constexpr size_t stage_bytes = key_region + val_region;
-    static constexpr size_t scratch_off = NSTAGE * stage_bytes;
-    static constexpr size_t meta_off = scratch_off + size_t(NW) * TILE * 4;
-    static constexpr size_t bar_off = meta_off + NSTAGE * sizeof(ShareMeta);
-    static constexpr size_t total = bar_off + 2 * NSTAGE * 8;
+    static constexpr size_t scratch_off = STAGES * stage_bytes;
+    static constexpr size_t meta_off = scratch_off + size_t(NWC) * TILE * 4;
+    static constexpr size_t bar_off = meta_off + STAGES * sizeof(ShareMeta);
+    static constexpr size_t total = bar_off + 2 * STAGES * 8;
+    static_assert(total + 1024 <= 227 * 1024, "stage buffers + scratch planes exceed the SM's shared memory");
     // 227 KiB of shared memory per SM, 1 KiB per CTA reserved by the system
     static constexpr int ctas_per_sm = (2 * (total + 1024) <= 227 * 1024) ? 2 : 1;
-    // registers per thread that keep ctas_per_sm CTAs of (NW + 1) warps resident (64 K registers per SM, allocation
-    // unit 8): stated to ptxas as the cap itself (__maxnreg__), because with __launch_bounds__ alone it settles on
-    // fewer registers than the SM offers and spills a word for the three-plane element type
-    static constexpr int max_regs = (65536 / ((NW + 1) * 32 * ctas_per_sm)) / 8 * 8;
+    // registers per thread that keep ctas_per_sm CTAs resident: the register file is 16 K registers per SM
+    // sub-partition and the warps of the resident CTAs are dealt round the four of them, so the bound is set by the
+    // sub-partition that gets ceil(warps / 4).  Stated to ptxas as the cap itself (__maxnreg__), because with
+    // __launch_bounds__ alone it settles on fewer registers than the SM offers and spills element data for the
+    // 64-bit key types.  (11 consumer warps + the producer = 3 warps per sub-partition at 168 registers.)
+    static constexpr int max_regs = (16384 / (((NWC + 1) * ctas_per_sm + 3) / 4 * 32)) / 8 * 8;
 };
 
 // ------------------------------------------------------------------ PTX wrappers (mbarrier, TMA)
@@ -179,7 +200,7 @@ partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict_
     const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     const unsigned long long s = (static_cast<unsigned long long>(blockIdx.x) * PART_THREADS + threadIdx.x) / G;
     if (s > num_shares) return;
-    const unsigned long long out0 = s * SH;
+    const unsigned long long out0 = s * Cfg<E>::SH;
     const unsigned long long a0 = out0 / (2 * L) * (2 * L);
     if (a0 >= n) { if (j == 0) splits[s] = 0; return; }
     const unsigned long long alen = min(L, n - a0);
@@ -343,7 +364,7 @@ __device__ __forceinline__ void aligned_superset(const unsigned long long g, con
 }
 
 template <class E>
-__global__ void __launch_bounds__(THREADS, Cfg<E>::ctas_per_sm)
+__global__ void __maxnreg__(Cfg<E>::max_regs)
 merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vin, void *__restrict__ kout,
                   uint32_t *__restrict__ vout, const uint32_t *__restrict__ splits, const unsigned long long n,
                   const unsigned long long L, const unsigned long long num_shares)
@@ -351,6 +372,7 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
     pdl_entry();
     using C = Cfg<E>;
     constexpr int KB = C::KB;
+    constexpr int SH = C::SH, NSTAGE = C::STAGES, NW = C::NWC;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint32_t *scratch_all = reinterpret_cast<uint32_t *>(smem_raw + C::scratch_off);
     ShareMeta *meta = reinterpret_cast<ShareMeta *>(smem_raw + C::meta_off);
@@ -365,7 +387,7 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
     if (threadIdx.x == 0) {
         for (int s = 0; s < NSTAGE; ++s) {
             mbar_init(&full[s], 1);
-            mbar_init(&empty[s], NW);
+            mbar_init(&empty[s], C::PAGES);      // one arrival per page of the share
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -379,6 +401,8 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
             const uint32_t ph = (it / NSTAGE) & 1u;
             unsigned char *kreg = smem_raw + st * C::stage_bytes;
             unsigned char *vreg = kreg + C::key_region;
+            // (waiting for the stage only after the split points are loaded -- later than here -- was measured: it
+            // changes nothing for the wide element types and costs the u32 kernel 10 %, 0.328 -> 0.363 ms per round)
             mbar_wait(&empty[st], ph ^ 1u);
             const unsigned long long out0 = s * SH;
             const int cnt = static_cast<int>(min(static_cast<unsigned long long>(SH), n - out0));
@@ -464,17 +488,22 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
     }
 
     // ============================== consumer warps
+    // Page g of this CTA's page sequence (share `it` of the CTA = pages PAGES * it .. + PAGES - 1) goes to warp
+    // g mod NWC.  A stage is released by the arrival of all its PAGES pages; a page a warp has not yet taken holds
+    // its stage back, so no barrier can run more than one phase ahead of a waiting warp.
     uint32_t *scratch = scratch_all + warp * TILE;
-    const int tile_off = warp * TILE;
-    unsigned int it = 0;
-    for (unsigned long long s = blockIdx.x; s < num_shares; s += gridDim.x, ++it) {
+    for (unsigned int g = warp;; g += NW) {
+        const unsigned int it = g / C::PAGES;
+        const unsigned long long s = blockIdx.x + static_cast<unsigned long long>(it) * gridDim.x;
+        if (s >= num_shares) break;
+        const int tile_off = static_cast<int>(g % C::PAGES) * TILE;
         const int st = it % NSTAGE;
         const uint32_t ph = (it / NSTAGE) & 1u;
         const unsigned char *kreg = smem_raw + st * C::stage_bytes;
         const unsigned char *vreg = kreg + C::key_region;
         mbar_wait(&full[st], ph);
         ShareMeta m = meta[st];
-        if (tile_off >= m.cnt) {            // ragged last share: nothing for this warp
+        if (tile_off >= m.cnt) {            // ragged last share: nothing on this page
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);
             continue;

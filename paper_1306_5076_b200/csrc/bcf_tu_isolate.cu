@@ -22,9 +22,9 @@ namespace bcf {
 namespace isolate {
 
 using E = Elem<1, false>;
-constexpr int NW = pipe::NW;
-constexpr int SH = pipe::SH;
-constexpr int NSTAGE = pipe::NSTAGE;
+constexpr int NW = pipe::Cfg<Elem<1, false>>::NWC;
+constexpr int SH = pipe::Cfg<Elem<1, false>>::SH;
+constexpr int NSTAGE = pipe::Cfg<Elem<1, false>>::STAGES;
 constexpr int THREADS = NW * 32;
 using C = pipe::Cfg<E>;
 constexpr size_t EXCLUSIVE_SMEM = 120 * 1024;      // more than half of the 227 KB an SM offers: one CTA per SM

@@ -9,7 +9,7 @@ namespace bcf {
 template <class E>
 bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len)
 {
-    const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
+    const unsigned long long shares = (n + pipe::Cfg<E>::SH - 1) / pipe::Cfg<E>::SH;
     const unsigned long long ull_n = n, ull_l = run_len;
     LaunchTimer t(BCF_KERNEL_PARTITION, c.s);
     // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
@@ -26,18 +26,18 @@ bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin
                              size_t n, size_t run_len)
 {
     using C = pipe::Cfg<E>;
-    const unsigned long long shares = (n + pipe::SH - 1) / pipe::SH;
+    const unsigned long long shares = (n + pipe::Cfg<E>::SH - 1) / pipe::Cfg<E>::SH;
     if (shares == 0) return BCF_OK;
     bcf_status st = ensure_dyn_smem<pipe::merge_pipe_kernel<E>>(c.dev, C::total);
     if (st != BCF_OK) return st;
-    if (2 * run_len > (size_t)pipe::SH) {
+    if (2 * run_len > (size_t)C::SH) {
         st = launch_partition_share<E>(c, kin, vin, splits, n, run_len);
         if (st != BCF_OK) return st;
     }
     LaunchTimer t(BCF_KERNEL_MERGE, c.s);
     const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * c.dev.num_sms;
     const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
-    return launch(c, pipe::merge_pipe_kernel<E>, blocks, pipe::THREADS, C::total, kin, vin, kout, vout,
+    return launch(c, pipe::merge_pipe_kernel<E>, blocks, C::THREADS, C::total, kin, vin, kout, vout,
                   static_cast<const uint32_t *>(splits), static_cast<unsigned long long>(n),
                   static_cast<unsigned long long>(run_len), shares);
 }
@@ -48,7 +48,7 @@ bool kernel_desc_pipe(int id, KernelDesc *k)
     switch (id) {
     case BCF_KID_PARTITION_SHARE_1: *k = {(const void *)pipe::partition_share_kernel<E, 1>, 0, pipe::PART_THREADS}; return true;
     case BCF_KID_PARTITION_SHARE_32: *k = {(const void *)pipe::partition_share_kernel<E, 32>, 0, pipe::PART_THREADS}; return true;
-    case BCF_KID_MERGE_PIPE: *k = {(const void *)pipe::merge_pipe_kernel<E>, pipe::Cfg<E>::total, pipe::THREADS}; return true;
+    case BCF_KID_MERGE_PIPE: *k = {(const void *)pipe::merge_pipe_kernel<E>, pipe::Cfg<E>::total, pipe::Cfg<E>::THREADS}; return true;
     }
     return false;
 }

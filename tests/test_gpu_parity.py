@@ -360,11 +360,7 @@ def test_error_codes(bcf):
 # Local memory (stack) bytes per thread the build is allowed to have, by (kernel, key type, value type).
 # makes "the data is not transferred to local memory" part of the method: every kernel must show 0 unless it is
 # listed here with the exact byte count (DESIGN.md section 4 names each entry and why it is not a data spill).
-LOCAL_BYTES_ALLOWED = {
-    # one scratch-plane address computed before the share loop, stored once and re-read once per share (STL/LDL
-    # of R2 in SASS); ptxas settles on 168 registers although the launch bound allows 224.  Not element data.
-    ("merge_pipe", 1, 1): 8,
-}
+LOCAL_BYTES_ALLOWED = {}      # none: every kernel of the build is at 0 bytes
 
 
 def test_every_launched_kernel_uses_no_local_memory(bcf):
