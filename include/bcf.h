@@ -139,7 +139,9 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
  *   rounds_per_pass merge rounds per read + write of the data: 1 (Lemma 2), 2 (four-run kernel
  *                   where it applies) or 0 = the library's choice.
  *   merge_impl      BCF_MERGE_IMPL_AUTO, or BCF_MERGE_IMPL_GENERIC = one warp per page with loads from global
- *                   memory (merge_kernel) even where the TMA-fed pipeline applies.
+ *                   memory (merge_kernel) even where the TMA-fed pipeline applies; BCF_MERGE_IMPL_BARRIER4 =
+ *                   four-run passes (rounds_per_pass = 2) always with the kernel that separates its two levels
+ *                   by CTA barriers (bcf_merge4.cuh) instead of the task-stream kernel (bcf_merge4s.cuh).
  *   partition_warp_search_max
  *                   largest number of share boundaries of a round searched with 32 lanes per boundary
  *                   (latency-bound case); above it one thread per boundary.  < 0 = default (4096).
@@ -150,7 +152,7 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
  *                   latency is a measurable share of the run time).
  */
 typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2, BCF_BASE_AUTO = 3 } bcf_base_case;
-typedef enum { BCF_MERGE_IMPL_AUTO = 0, BCF_MERGE_IMPL_GENERIC = 1 } bcf_merge_impl;
+typedef enum { BCF_MERGE_IMPL_AUTO = 0, BCF_MERGE_IMPL_GENERIC = 1, BCF_MERGE_IMPL_BARRIER4 = 2 } bcf_merge_impl;
 typedef enum { BCF_LAUNCH_AUTO = 0, BCF_LAUNCH_PLAIN = 1, BCF_LAUNCH_PDL = 2 } bcf_launch_mode;
 typedef struct bcf_options {
     uint32_t struct_size;
@@ -426,7 +428,8 @@ typedef enum {
     BCF_KID_MERGE4_PIPE = 11,
     BCF_KID_MERGE_PAGEWISE = 12,
     BCF_KID_MERGE_PIECES = 13,
-    BCF_KID_COUNT = 14
+    BCF_KID_MERGE4_STREAM = 14,
+    BCF_KID_COUNT = 15
 } bcf_kernel_id;
 const char *bcf_kernel_name(int kernel_id);
 bcf_status bcf_kernel_info(int kernel_id, bcf_key_t kt, bcf_val_t vt, int *regs_per_thread,

@@ -38,6 +38,7 @@ from .binding import (  # noqa: F401
     profile_dropped,
     MERGE_IMPL_AUTO,
     MERGE_IMPL_GENERIC,
+    MERGE_IMPL_BARRIER4,
     LAUNCH_AUTO,
     LAUNCH_PLAIN,
     LAUNCH_PDL,

@@ -15,9 +15,9 @@ KERNEL_CLASSES = ("tile_sort", "partition", "merge", "merge_pagewise")
 # bcf_kernel_id (include/bcf.h): every kernel the library can launch
 KERNEL_IDS = ("tile_sort", "tile_mergesort", "long_tile_2", "long_tile_4", "long_tile_8", "partition", "merge",
               "partition_share_1", "partition_share_32", "merge_pipe", "partition4", "merge4_pipe", "merge_pagewise",
-              "merge_pieces")
+              "merge_pieces", "merge4_stream")
 BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES, BASE_AUTO = 0, 1, 2, 3
-MERGE_IMPL_AUTO, MERGE_IMPL_GENERIC = 0, 1
+MERGE_IMPL_AUTO, MERGE_IMPL_GENERIC, MERGE_IMPL_BARRIER4 = 0, 1, 2
 LAUNCH_AUTO, LAUNCH_PLAIN, LAUNCH_PDL = 0, 1, 2
 
 

@@ -83,11 +83,12 @@ bool resolve_options(const bcf_options *o, Opt *r)
     if (o->struct_size < sizeof(bcf_options)) return false;
     if (o->base_case < BCF_BASE_SHEARSORT || o->base_case > BCF_BASE_AUTO) return false;
     if (o->rounds_per_pass < 0 || o->rounds_per_pass > 2) return false;
-    if (o->merge_impl != BCF_MERGE_IMPL_AUTO && o->merge_impl != BCF_MERGE_IMPL_GENERIC) return false;
+    if (o->merge_impl < BCF_MERGE_IMPL_AUTO || o->merge_impl > BCF_MERGE_IMPL_BARRIER4) return false;
     if (o->launch_mode < BCF_LAUNCH_AUTO || o->launch_mode > BCF_LAUNCH_PDL) return false;
     r->base_case = o->base_case;
     if (o->rounds_per_pass) r->rounds_per_pass = o->rounds_per_pass;
     r->generic_merge = o->merge_impl == BCF_MERGE_IMPL_GENERIC;
+    r->merge4_barrier = o->merge_impl == BCF_MERGE_IMPL_BARRIER4;
     if (o->partition_warp_search_max >= 0) r->warp_search_max = static_cast<unsigned long long>(o->partition_warp_search_max);
     r->launch_mode = o->launch_mode;
     return true;
@@ -956,7 +957,7 @@ const char *bcf_kernel_name(int kernel_id)
         "tile_sort_kernel", "tile_mergesort_kernel", "long_tile_sort_kernel<h=2>", "long_tile_sort_kernel<h=4>",
         "long_tile_sort_kernel<h=8>", "partition_kernel", "merge_kernel", "partition_share_kernel<G=1>",
         "partition_share_kernel<G=32>", "merge_pipe_kernel", "partition4_kernel", "merge4_pipe_kernel",
-        "pagewise_merge_kernel", "merge_pieces_kernel"};
+        "pagewise_merge_kernel", "merge_pieces_kernel", "merge4_stream_kernel"};
     return (kernel_id >= 0 && kernel_id < BCF_KID_COUNT) ? names[kernel_id] : nullptr;
 }
 

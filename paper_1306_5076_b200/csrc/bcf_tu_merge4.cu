@@ -2,6 +2,7 @@
 // selection + two merge rounds per read + write of the data.
 #include "bcf_internal.cuh"
 #include "bcf_merge4.cuh"
+#include "bcf_merge4s.cuh"
 
 namespace bcf {
 
@@ -36,6 +37,19 @@ bcf_status launch_merge4(const Call &c, const void *kin, const uint32_t *vin, vo
         if (4 * run_len > (size_t)pipe4::SH) {
             st = launch_partition4<E>(c, kin, vin, splits, n, run_len, shares + 1);
             if (st != BCF_OK) return st;
+            // shares that cut through the runs: the task-stream kernel (no CTA barrier between the two levels)
+            if constexpr (pipe4s::Cfg4s<E>::fits) {
+                if (!c.opt.merge4_barrier) {
+                    using S = pipe4s::Cfg4s<E>;
+                    st = ensure_dyn_smem<pipe4s::merge4_stream_kernel<E>>(c.dev, S::total);
+                    if (st != BCF_OK) return st;
+                    LaunchTimer t(BCF_KERNEL_MERGE, c.s);
+                    const unsigned long long sms = c.dev.num_sms;
+                    return launch(c, pipe4s::merge4_stream_kernel<E>, static_cast<unsigned>(shares < sms ? shares : sms), pipe4s::THREADS,
+                                  S::total, kin, vin, kout, vout, reinterpret_cast<const uint4 *>(splits),
+                                  static_cast<unsigned long long>(n), static_cast<unsigned long long>(run_len), shares);
+                }
+            }
         }
         LaunchTimer t(BCF_KERNEL_MERGE, c.s);
         const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * c.dev.num_sms;
@@ -54,6 +68,13 @@ bool kernel_desc_merge4(int id, KernelDesc *k)
     case BCF_KID_MERGE4_PIPE:
         if constexpr (pipe4::Cfg4<E>::fits) {
             *k = {(const void *)pipe4::merge4_pipe_kernel<E>, pipe4::Cfg4<E>::total, pipe4::THREADS};
+            return true;
+        } else {
+            return false;
+        }
+    case BCF_KID_MERGE4_STREAM:
+        if constexpr (pipe4s::Cfg4s<E>::fits) {
+            *k = {(const void *)pipe4s::merge4_stream_kernel<E>, pipe4s::Cfg4s<E>::total, pipe4s::THREADS};
             return true;
         } else {
             return false;

@@ -20,11 +20,16 @@ def bcf():
     return m
 
 
-@pytest.fixture(params=[1, 2], ids=["1round", "2rounds"])
+# bcf_options of the pass structures of the merging phase
+RPP = {1: {"rounds_per_pass": 1}, 2: {"rounds_per_pass": 2}, 3: {"rounds_per_pass": 2, "merge_impl": 2}}
+
+
+@pytest.fixture(params=[1, 2, 3], ids=["1round", "2rounds", "2rounds-barrier"])
 def rpp(request):
-    """Both pass structures of the merging phase, passed per call in bcf_options: one round per pass
-    (Lemma 2) and two rounds per pass (four-run kernel); the result must be the same unique
-    sorted output."""
+    """The pass structures of the merging phase, passed per call in bcf_options: one round per pass
+    (Lemma 2), two rounds per pass (four-run kernels: the task-stream kernel where it applies), and
+    two rounds per pass with the barrier version of the four-run kernel everywhere; the result must be the same
+    unique sorted output."""
     return request.param
 
 
@@ -227,7 +232,7 @@ def test_merge_runs_matches_oracle(bcf, kind, n, run_len, rpp):
     else:
         keys, vals = workloads.sorted_runs(keys, run_len, vals)
     dk, dv = dev(keys), dev(vals)
-    out = bcf.merge_runs(dk, run_len, dv, opts={"rounds_per_pass": rpp})
+    out = bcf.merge_runs(dk, run_len, dv, opts={**RPP[rpp]})
     want = oracle.merge_runs(keys, run_len, vals)
     if vals is None:
         assert np.array_equal(host(out, keys), want)
@@ -236,10 +241,19 @@ def test_merge_runs_matches_oracle(bcf, kind, n, run_len, rpp):
     assert np.array_equal(host(dk, keys), keys)          # the input is not modified
 
 
+@pytest.mark.parametrize("n,run_len", [(5_000_000, 1 << 13), ((1 << 22) + 777, 1 << 14), (1 << 23, 1 << 21)])
+def test_four_run_passes_many_shares_per_cta(bcf, n, run_len, rpp):
+    """More shares than SMs: every CTA of the persistent four-run kernels works through several shares, so the
+    stage and X-Y buffers are refilled and every mbarrier runs through several phases (bcf_merge4s.cuh)."""
+    keys = workloads.sorted_runs(make("u32", n, seed=n % 1000)[0], run_len)
+    out = bcf.merge_runs(dev(keys), run_len, opts={**RPP[rpp]})
+    assert np.array_equal(host(out, keys), oracle.merge_runs(keys, run_len))
+
+
 @pytest.mark.parametrize("k", [2, 64, 1024])
 def test_merge_runs_config5b_shape(bcf, k, rpp):
     keys, run_len = workloads.cfg5b_merge_runs_u32(k, n=1 << 18)
-    out = bcf.merge_runs(dev(keys), run_len, opts={"rounds_per_pass": rpp})
+    out = bcf.merge_runs(dev(keys), run_len, opts={**RPP[rpp]})
     assert np.array_equal(host(out, keys), oracle.merge_runs(keys, run_len))
 
 
@@ -281,7 +295,7 @@ def test_merge_runs_pagewise_matches_oracle(bcf, kind, n, run_len):
 def test_sort_matches_oracle(bcf, kind, n, rpp, base):
     keys, vals = make(kind, n, seed=n, dup=(n % 3 == 0))
     dk, dv = dev(keys), dev(vals)
-    bcf.sort(dk, dv, opts={"rounds_per_pass": rpp, "base_case": base})
+    bcf.sort(dk, dv, opts={**RPP[rpp], "base_case": base})
     want = oracle.sort_full(keys, vals)
     assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
 
@@ -295,7 +309,7 @@ def test_sort_launch_modes(bcf, n, rpp, launch_mode):
         dk, dv = dev(keys), dev(vals)
         for _ in range(3):                                   # back-to-back calls on one stream
             dk.copy_(dev(keys))
-            bcf.sort(dk, dv if vals is None else dv.copy_(dev(vals)), opts={"rounds_per_pass": rpp, "launch_mode": launch_mode})
+            bcf.sort(dk, dv if vals is None else dv.copy_(dev(vals)), opts={**RPP[rpp], "launch_mode": launch_mode})
         want = oracle.sort_full(keys, vals)
         assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
 
@@ -304,18 +318,18 @@ def test_sort_launch_modes(bcf, n, rpp, launch_mode):
 def test_sort_config4_distributions(bcf, dist, rpp, base):
     keys = workloads.cfg4_sort_u32(dist, n=(1 << 18) + 1000)
     d = dev(keys)
-    bcf.sort(d, opts={"rounds_per_pass": rpp, "base_case": base})
+    bcf.sort(d, opts={**RPP[rpp], "base_case": base})
     assert np.array_equal(host(d, keys), oracle.sort_full(keys))
 
 
 def test_sort_config3_and_5a_shapes(bcf, rpp):
     keys = workloads.cfg3_sort_u32(n=1 << 19)
     d = dev(keys)
-    bcf.sort(d, opts={"rounds_per_pass": rpp})
+    bcf.sort(d, opts={**RPP[rpp]})
     assert np.array_equal(host(d, keys), oracle.sort_full(keys))
     k, v = workloads.cfg5a_sort_u64_u32(n=(1 << 18) + 3)
     dk, dv = dev(k), dev(v)
-    bcf.sort(dk, dv, opts={"rounds_per_pass": rpp})
+    bcf.sort(dk, dv, opts={**RPP[rpp]})
     wk, wv = oracle.sort_full(k, v)
     assert np.array_equal(host(dk, k), wk) and np.array_equal(host(dv, v), wv)
 
@@ -364,7 +378,7 @@ LOCAL_BYTES_ALLOWED = {}      # none: every kernel of the build is at 0 bytes
 
 
 def test_every_launched_kernel_uses_no_local_memory(bcf):
-    """All 14 kernels x 4 element types (those that exist): cudaFuncGetAttributes().localSizeBytes == 0."""
+    """All 15 kernels x 4 element types (those that exist): cudaFuncGetAttributes().localSizeBytes == 0."""
     seen = 0
     for kid in bcf.KERNEL_IDS:
         for kt in (0, 1):
@@ -373,12 +387,13 @@ def test_every_launched_kernel_uses_no_local_memory(bcf):
                     info = bcf.kernel_info(kid, kt, vt)
                 except bcf.BcfError as e:
                     assert e.name == "BCF_ERR_INVALID_ARG"
-                    assert (kid == "merge4_pipe" and (kt, vt) == (1, 1)) or (kid == "merge_pieces" and vt == 1), (kid, kt, vt)
+                    assert ((kid == "merge4_pipe" and (kt, vt) == (1, 1)) or (kid == "merge_pieces" and vt == 1) or
+                            (kid == "merge4_stream" and (kt, vt) != (0, 0))), (kid, kt, vt)
                     continue
                 seen += 1
                 assert info["local_bytes_per_thread"] == LOCAL_BYTES_ALLOWED.get((kid, kt, vt), 0), (kid, kt, vt, info)
                 assert info["ctas_per_sm"] >= 1, (kid, kt, vt, info)
-    assert seen == 14 * 4 - 1 - 2
+    assert seen == 15 * 4 - 1 - 2 - 3
 
 
 def test_options_are_per_call_and_validated(bcf):
