@@ -894,7 +894,7 @@ bcf_status bcf_debug_merge_round_isolated(const void *d_keys_in, void *d_keys_ou
     if (st != BCF_OK) return st;
     ProfileGroup profile_group(stream);
     uint32_t *splits = static_cast<uint32_t *>(d_workspace);
-    st = launch_partition_share<E_U32>(c, d_keys_in, nullptr, splits, n, run_len);
+    st = launch_partition_share<E_U32>(c, d_keys_in, nullptr, splits, n, run_len, isolated_share());
     if (st != BCF_OK) return st;
     return launch_isolated_merge_round(c, static_cast<const uint32_t *>(d_keys_in), static_cast<uint32_t *>(d_keys_out), splits, n,
                                        run_len, exclusive);

@@ -176,8 +176,10 @@ bcf_status launch_pagewise(const Call &c, const void *kin, const uint32_t *vin, 
 template <class E>
 bool kernel_desc_merge(int id, KernelDesc *k);
 // bcf_tu_pipe.cu
+// share = 0: the share size of the production merge kernel for E
 template <class E>
-bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len);
+bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len,
+                                  size_t share);
 template <class E>
 bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits,
                              size_t n, size_t run_len);
@@ -210,6 +212,7 @@ bcf_status launch_colored_scan(const Call &c, const uint32_t *values, const uint
                                uint32_t *partial, uint32_t *out);
 
 // bcf_tu_isolate.cu: the bank-conflict isolation experiment (debug entry points of include/bcf.h)
+size_t isolated_share();        // share size of the experiment's merge round
 bcf_status launch_isolated_merge_round(const Call &c, const uint32_t *kin, uint32_t *kout, const uint32_t *splits, size_t n,
                                        size_t run_len, int exclusive);
 bcf_status launch_isolated_tile_mergesort(const Call &c, uint32_t *keys, size_t num_tiles, int exclusive);

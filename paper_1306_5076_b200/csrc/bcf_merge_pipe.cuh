@@ -63,14 +63,20 @@ struct ShareMeta {
 #ifndef BCF_PIPE_NWC12
 #define BCF_PIPE_NWC12 11    // consumer warps, 12-byte elements
 #endif
+#ifndef BCF_PIPE_PAGES4
+#define BCF_PIPE_PAGES4 16   // pages per share, 4-byte elements
+#endif
+#ifndef BCF_PIPE_NWC4
+#define BCF_PIPE_NWC4 19     // consumer warps, 4-byte elements
+#endif
 template <class E>
 struct Cfg {
     static constexpr int KB = E::KEY_BYTES;
     static constexpr int EB = KB + (E::HAS_VAL ? 4 : 0);
-    static constexpr int PAGES = EB >= 12 ? 4 : 8;            // pages per share
+    static constexpr int PAGES = EB >= 12 ? 4 : (EB == 4 ? BCF_PIPE_PAGES4 : 8);   // pages per share
     static constexpr int SH = PAGES * TILE;                    // outputs per share
     static constexpr int STAGES = EB >= 12 ? 3 : 2;
-    static constexpr int NWC = EB == 4 ? 8 : (EB == 8 ? BCF_PIPE_NWC8 : BCF_PIPE_NWC12);
+    static constexpr int NWC = EB == 4 ? BCF_PIPE_NWC4 : (EB == 8 ? BCF_PIPE_NWC8 : BCF_PIPE_NWC12);
     static constexpr int THREADS = (NWC + 1) * 32;
     static constexpr size_t key_region = size_t(SH) * KB + REGION_SLACK;
     static constexpr size_t val_region = E::HAS_VAL ? size_t(SH) * 4 + REGION_SLACK : 0;
@@ -190,17 +196,22 @@ __device__ __forceinline__ int corank_smem(const unsigned char *kreg, const unsi
 // bandwidth-bound and the plain binary search (G = 1) is faster (measured).
 // Only launched for rounds with 2 L > SH.
 constexpr int PART_THREADS = 128;
+#ifndef BCF_PART_PROBES
+#define BCF_PART_PROBES 2
+#endif
+constexpr int PART_PROBES = BCF_PART_PROBES;
 template <class E, int G>
 __global__ void __launch_bounds__(PART_THREADS)
 partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
-                       const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)
+                       const unsigned long long n, const unsigned long long L, const unsigned long long num_shares,
+                       const unsigned long long share)
 {
     pdl_entry();
     const int j = threadIdx.x % G;                       // lane inside the group
     const unsigned gmask = (G == 32) ? 0xFFFFFFFFu : (((1u << G) - 1u) << ((threadIdx.x & 31) / G * G));
     const unsigned long long s = (static_cast<unsigned long long>(blockIdx.x) * PART_THREADS + threadIdx.x) / G;
     if (s > num_shares) return;
-    const unsigned long long out0 = s * Cfg<E>::SH;
+    const unsigned long long out0 = s * share;
     const unsigned long long a0 = out0 / (2 * L) * (2 * L);
     if (a0 >= n) { if (j == 0) splits[s] = 0; return; }
     const unsigned long long alen = min(L, n - a0);
@@ -210,10 +221,23 @@ partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict_
     unsigned long long lo = d > blen ? d - blen : 0ull;
     unsigned long long hi = min(d, alen);
     if constexpr (G == 1) {
+        // one thread per boundary, PART_PROBES probes per round: the probes of a round are independent loads, so a
+        // round costs one memory latency and narrows the range PART_PROBES-fold (14 dependent rounds instead of the
+        // 27 of a binary search for a pair of 2^27-element runs; the launch is latency-bound)
         while (lo < hi) {
-            const unsigned long long mid = (lo + hi) >> 1;
-            if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
-            else hi = mid;
+            const unsigned long long step = (hi - lo + PART_PROBES - 1) / PART_PROBES;
+            bool le[PART_PROBES];
+#pragma unroll
+            for (int q = 0; q < PART_PROBES; ++q) {
+                const unsigned long long mid = lo + q * step;
+                le[q] = mid < hi && elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid));
+            }
+            unsigned long long c = 0;      // the predicate is monotone: the probes that hold are a prefix
+#pragma unroll
+            for (int q = 0; q < PART_PROBES; ++q) c += le[q] ? 1u : 0u;
+            const unsigned long long nlo = c ? lo + (c - 1) * step + 1 : lo;
+            hi = min(hi, lo + c * step);
+            lo = nlo;
         }
     } else {
         while (lo < hi) {

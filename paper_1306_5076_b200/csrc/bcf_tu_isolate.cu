@@ -22,11 +22,19 @@ namespace bcf {
 namespace isolate {
 
 using E = Elem<1, false>;
-constexpr int NW = pipe::Cfg<Elem<1, false>>::NWC;
-constexpr int SH = pipe::Cfg<Elem<1, false>>::SH;
-constexpr int NSTAGE = pipe::Cfg<Elem<1, false>>::STAGES;
+// the shape of the experiment is fixed here, whatever the production kernel uses: shares of 8 pages, one page per warp,
+// two stage buffers (profiles/r2_conflict_isolation.md was measured with exactly this)
+constexpr int NW = 8;
+constexpr int SH = NW * TILE;
+constexpr int NSTAGE = 2;
 constexpr int THREADS = NW * 32;
-using C = pipe::Cfg<E>;
+struct C {
+    static constexpr size_t stage_bytes = size_t(SH) * 4 + pipe::REGION_SLACK;
+    static constexpr size_t scratch_off = NSTAGE * stage_bytes;
+    static constexpr size_t meta_off = scratch_off + size_t(NW) * TILE * 4;
+    static constexpr size_t bar_off = meta_off + NSTAGE * sizeof(pipe::ShareMeta);
+    static constexpr size_t total = bar_off + NSTAGE * 8;
+};
 constexpr size_t EXCLUSIVE_SMEM = 120 * 1024;      // more than half of the 227 KB an SM offers: one CTA per SM
 
 // One merge round on u32 keys, runs of L = 1024 * 2^k >= 8192, n a multiple of 8192: each CTA merges NSTAGE shares.
@@ -171,6 +179,8 @@ tile_mergesort_isolated_kernel(uint32_t *__restrict__ keys, const size_t num_til
 }
 
 }  // namespace isolate
+
+size_t isolated_share() { return isolate::SH; }
 
 bcf_status launch_isolated_merge_round(const Call &c, const uint32_t *kin, uint32_t *kout, const uint32_t *splits, size_t n,
                                        size_t run_len, int exclusive)

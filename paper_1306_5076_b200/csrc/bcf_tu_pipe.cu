@@ -7,18 +7,21 @@ namespace bcf {
 
 // split points of the share boundaries of one round (only rounds with 2 L > SH need them)
 template <class E>
-bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len)
+bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len,
+                                  size_t share)
 {
-    const unsigned long long shares = (n + pipe::Cfg<E>::SH - 1) / pipe::Cfg<E>::SH;
+    if (share == 0) share = pipe::Cfg<E>::SH;
+    const unsigned long long shares = (n + share - 1) / share;
+    const unsigned long long ull_share = share;
     const unsigned long long ull_n = n, ull_l = run_len;
     LaunchTimer t(BCF_KERNEL_PARTITION, c.s);
     // few boundaries: latency-bound, 32 lanes per boundary; many: bandwidth-bound, one thread each
     if (shares + 1 <= c.opt.warp_search_max) {
         const unsigned blocks = static_cast<unsigned>(((shares + 1) * 32 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-        return launch(c, pipe::partition_share_kernel<E, 32>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
+        return launch(c, pipe::partition_share_kernel<E, 32>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares, ull_share);
     }
     const unsigned blocks = static_cast<unsigned>((shares + 1 + pipe::PART_THREADS - 1) / pipe::PART_THREADS);
-    return launch(c, pipe::partition_share_kernel<E, 1>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares);
+    return launch(c, pipe::partition_share_kernel<E, 1>, blocks, pipe::PART_THREADS, 0, kin, vin, splits, ull_n, ull_l, shares, ull_share);
 }
 
 template <class E>
@@ -31,7 +34,7 @@ bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin
     bcf_status st = ensure_dyn_smem<pipe::merge_pipe_kernel<E>>(c.dev, C::total);
     if (st != BCF_OK) return st;
     if (2 * run_len > (size_t)C::SH) {
-        st = launch_partition_share<E>(c, kin, vin, splits, n, run_len);
+        st = launch_partition_share<E>(c, kin, vin, splits, n, run_len, 0);
         if (st != BCF_OK) return st;
     }
     LaunchTimer t(BCF_KERNEL_MERGE, c.s);
@@ -53,16 +56,16 @@ bool kernel_desc_pipe(int id, KernelDesc *k)
     return false;
 }
 
-template bcf_status launch_partition_share<E_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
+template bcf_status launch_partition_share<E_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U32>(int, KernelDesc *);
-template bcf_status launch_partition_share<E_U32_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
+template bcf_status launch_partition_share<E_U32_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U32_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U32_U32>(int, KernelDesc *);
-template bcf_status launch_partition_share<E_U64>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
+template bcf_status launch_partition_share<E_U64>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U64>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U64>(int, KernelDesc *);
-template bcf_status launch_partition_share<E_U64_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t);
+template bcf_status launch_partition_share<E_U64_U32>(const Call &, const void *, const uint32_t *, uint32_t *, size_t, size_t, size_t);
 template bcf_status launch_merge_pipe<E_U64_U32>(const Call &, const void *, const uint32_t *, void *, uint32_t *, uint32_t *, size_t, size_t);
 template bool kernel_desc_pipe<E_U64_U32>(int, KernelDesc *);
 
