@@ -68,12 +68,9 @@ bcf_status current_device(Dev *d)
 #ifndef BCF_DEFAULT_ROUNDS_PER_PASS
 #define BCF_DEFAULT_ROUNDS_PER_PASS 1
 #endif
-// BCF_LAUNCH_AUTO: programmatic dependent launches below this many elements.  Measured on B200:
-// they hide the launch latency between the ~2 launches of every merge round, which is 27 % of a 2^20-key sort and
-// 11 % of a 2^24-key sort, but cost 2 % at 2^28 keys where every launch runs for a third of a millisecond.
-#ifndef BCF_PDL_AUTO_MAX_N
-#define BCF_PDL_AUTO_MAX_N (size_t(1) << 26)
-#endif
+// BCF_LAUNCH_AUTO = programmatic dependent launches at every size.  Measured on B200: they hide
+// the launch latency between the ~2 launches of every merge round, which is 27 % of a 2^20-key sort, 11 % of a
+// 2^24-key sort and still 1 % at 2^28 keys (6.89 against 6.95 ms; r2).
 
 bool resolve_options(const bcf_options *o, Opt *r)
 {
@@ -97,7 +94,8 @@ bool resolve_options(const bcf_options *o, Opt *r)
 // launch mode of a call that works on n elements
 inline void resolve_launch_mode(Opt *o, size_t n)
 {
-    o->pdl = o->launch_mode == BCF_LAUNCH_PDL || (o->launch_mode == BCF_LAUNCH_AUTO && n < BCF_PDL_AUTO_MAX_N);
+    (void)n;
+    o->pdl = o->launch_mode != BCF_LAUNCH_PLAIN;
 }
 
 bool overlap(const void *a, size_t an, const void *b, size_t bn)

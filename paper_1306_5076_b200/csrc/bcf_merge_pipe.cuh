@@ -8,8 +8,8 @@
 // here every CTA takes an equal SHARE of the output of a round instead (north_star: "split-point
 // search so each CTA gets an equal share of output"):
 //
-//   share      = SH = PAGES * 1024 consecutive outputs of the round (PAGES = 8; 4 for twelve-byte elements), one
-//                page (sub-tile) of 1024 outputs per consumer warp at a time
+//   share      = SH = PAGES * 1024 consecutive outputs of the round (PAGES = 16 / 4 / 8 for 4- / 8- / 12-byte
+//                elements), one page (sub-tile) of 1024 outputs per consumer warp at a time
 //   producer   = one extra warp.  For share s it works out which input the share needs
 //                  - run length 2L <= SH: the share's own input range (whole pairs),
 //                  - otherwise: A[I0, I1) and B[D0 - I0, D1 - I1) from the global split points
@@ -17,8 +17,8 @@
 //                and issues cp.async.bulk (TMA, UBLKCP) copies global -> shared that complete on an
 //                mbarrier.  NSTAGE stage buffers: the copies of share i+1 are in flight while the
 //                consumers work on share i; no load ever occupies a register or an LSU slot.
-//   consumers  = NWC warps (8 / 15 / 11 for 4- / 8- / 12-byte elements, Cfg below) that take the pages of the
-//                CTA's shares round robin.  Each finds the two split points of its own sub-tile INSIDE shared memory
+//   consumers  = NWC warps (16 / 12 / 8 for 4- / 8- / 12-byte elements, Cfg below), each owning one page position
+//                of the shares it works on.  Each finds the two split points of its own sub-tile INSIDE shared memory
 //                with a conflict-free 32-ary search (corank_smem), reads its 1024 elements from the
 //                stage buffer straight into the column layout (word address consecutive across
 //                lanes: conflict-free for any offset), releases the stage, and runs SHEARSORT-MERGE
@@ -50,33 +50,49 @@ struct ShareMeta {
     int pad;
 };
 
-// Shape of the kernel per element type.  A share is PAGES pages of 1024 outputs; NWC consumer warps take the pages
-// of the CTA's shares round robin (page g of the CTA's page sequence goes to warp g mod NWC), so the number of
-// warps is free of the share size: 4-byte elements keep 8 warps = 8 pages and two CTAs per SM; the wider element
-// types cost 2.5-10 times the ALU work per comparator and run ONE CTA per SM (the stage buffers fill it), where 8
-// warps -- two per SM sub-partition -- left the ALU pipe 40 % idle waiting on fixed-latency dependences
-// (profiles/r2a_merge_kv_full.md); they get as many warps as the register file holds, and twelve-byte elements
-// shares of 4 pages in 3 stage buffers so that the warps' scratch planes still fit.
-#ifndef BCF_PIPE_NWC8
-#define BCF_PIPE_NWC8 15     // consumer warps, 8-byte elements
-#endif
-#ifndef BCF_PIPE_NWC12
-#define BCF_PIPE_NWC12 11    // consumer warps, 12-byte elements
-#endif
+// Shape of the kernel per element type.  A share is PAGES pages of 1024 outputs in one of STAGES stage buffers; the
+// NWC consumer warps form GROUPS = NWC / PAGES groups of PAGES warps, warp w owning page w mod PAGES of the shares
+// of its group:
+//   GROUPS = 1      every warp takes its page of EVERY share of the CTA (4-byte elements: 16 warps, 16 pages);
+//   GROUPS = STAGES group j takes the shares that land in stage buffer j (every STAGES-th share of the CTA), so
+//                   more warps than pages of a share can be busy (8-byte elements: 3 stage buffers of 4 pages, 12
+//                   warps at 128 registers: 0.216 -> 0.185 ms per round at 2^26 (u32,u32) pairs against 8 warps on
+//                   2 buffers of 8 pages).  Twelve-byte elements need 168 registers, which allows 8 consumer warps
+//                   either way; one group on shares of 8 pages is the faster shape for them.
+// No other assignment is allowed, for the sake of the barriers: an mbarrier wait names the phase it waits for by
+// ONE parity bit, which is sound only if the waiting warp took part in the previous phase of that barrier (otherwise
+// the barrier may be one phase behind -- the wait passes on stale data -- or two phases ahead -- the wait never
+// returns).  In both shapes a warp waits on a stage buffer exactly in the phases in which it reads a page from it.
+// (A first version dealt pages round robin to 19 / 15 / 11 warps; it was 0.2-6 % faster and crashed about once in
+// ten runs of a 2^28-key sort on exactly this.)
 #ifndef BCF_PIPE_PAGES4
 #define BCF_PIPE_PAGES4 16   // pages per share, 4-byte elements
 #endif
-#ifndef BCF_PIPE_NWC4
-#define BCF_PIPE_NWC4 19     // consumer warps, 4-byte elements
+#ifndef BCF_PIPE_PAGES8
+#define BCF_PIPE_PAGES8 4    // pages per share, 8-byte elements
+#endif
+#ifndef BCF_PIPE_STAGES8
+#define BCF_PIPE_STAGES8 3
+#endif
+#ifndef BCF_PIPE_PAGES12
+#define BCF_PIPE_PAGES12 8   // pages per share, 12-byte elements
+#endif
+#ifndef BCF_PIPE_STAGES12
+#define BCF_PIPE_STAGES12 2
+#endif
+#ifndef BCF_PIPE_GROUPS12
+#define BCF_PIPE_GROUPS12 1  // 8 warps at 168 registers; two groups on shares of 4 pages measured slower (0.322 against 0.314 ms)
 #endif
 template <class E>
 struct Cfg {
     static constexpr int KB = E::KEY_BYTES;
     static constexpr int EB = KB + (E::HAS_VAL ? 4 : 0);
-    static constexpr int PAGES = EB >= 12 ? 4 : (EB == 4 ? BCF_PIPE_PAGES4 : 8);   // pages per share
+    static constexpr int PAGES = EB == 4 ? BCF_PIPE_PAGES4 : (EB == 8 ? BCF_PIPE_PAGES8 : BCF_PIPE_PAGES12);   // pages per share
     static constexpr int SH = PAGES * TILE;                    // outputs per share
-    static constexpr int STAGES = EB >= 12 ? 3 : 2;
-    static constexpr int NWC = EB == 4 ? BCF_PIPE_NWC4 : (EB == 8 ? BCF_PIPE_NWC8 : BCF_PIPE_NWC12);
+    static constexpr int STAGES = EB == 4 ? 2 : (EB == 8 ? BCF_PIPE_STAGES8 : BCF_PIPE_STAGES12);
+    static constexpr int GROUPS = EB == 4 ? 1 : (EB == 8 ? STAGES : BCF_PIPE_GROUPS12);
+    static_assert(GROUPS == 1 || GROUPS == STAGES, "see above: a warp must take part in every phase it waits on");
+    static constexpr int NWC = GROUPS * PAGES;
     static constexpr int THREADS = (NWC + 1) * 32;
     static constexpr size_t key_region = size_t(SH) * KB + REGION_SLACK;
     static constexpr size_t val_region = E::HAS_VAL ? size_t(SH) * 4 + REGION_SLACK : 0;
@@ -92,7 +108,7 @@ struct Cfg {
     // sub-partition and the warps of the resident CTAs are dealt round the four of them, so the bound is set by the
     // sub-partition that gets ceil(warps / 4).  Stated to ptxas as the cap itself (__maxnreg__), because with
     // __launch_bounds__ alone it settles on fewer registers than the SM offers and spills element data for the
-    // 64-bit key types.  (11 consumer warps + the producer = 3 warps per sub-partition at 168 registers.)
+    // 64-bit key types.
     static constexpr int max_regs = (16384 / (((NWC + 1) * ctas_per_sm + 3) / 4 * 32)) / 8 * 8;
 };
 
@@ -512,15 +528,12 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
     }
 
     // ============================== consumer warps
-    // Page g of this CTA's page sequence (share `it` of the CTA = pages PAGES * it .. + PAGES - 1) goes to warp
-    // g mod NWC.  A stage is released by the arrival of all its PAGES pages; a page a warp has not yet taken holds
-    // its stage back, so no barrier can run more than one phase ahead of a waiting warp.
+    // warp w: page w mod PAGES of the shares of group w / PAGES (Cfg above)
     uint32_t *scratch = scratch_all + warp * TILE;
-    for (unsigned int g = warp;; g += NW) {
-        const unsigned int it = g / C::PAGES;
+    const int tile_off = (warp % C::PAGES) * TILE;
+    for (unsigned int it = warp / C::PAGES;; it += C::GROUPS) {
         const unsigned long long s = blockIdx.x + static_cast<unsigned long long>(it) * gridDim.x;
         if (s >= num_shares) break;
-        const int tile_off = static_cast<int>(g % C::PAGES) * TILE;
         const int st = it % NSTAGE;
         const uint32_t ph = (it / NSTAGE) & 1u;
         const unsigned char *kreg = smem_raw + st * C::stage_bytes;

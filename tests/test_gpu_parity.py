@@ -595,3 +595,28 @@ def test_sort_is_deterministic_under_repetition(bcf):
                 dk, dv = dev(keys), dev(vals)
                 bcf.sort(dk, dv, opts=o)
                 assert_same(host(dk, keys), None if vals is None else host(dv, vals), want, vals)
+
+
+@pytest.mark.parametrize("kind,logn", [("u32", 24), ("u32u32", 23), ("u64u32", 23)])
+def test_persistent_merge_kernels_are_deterministic_over_many_shares(bcf, kind, logn):
+    """Every CTA of the persistent merge kernels works through several shares here, so their stage buffers are
+    refilled and their mbarriers run through many phases (a warp that waits on a phase it did not take part in --
+    bcf_merge_pipe.cuh, Cfg -- showed as an illegal address about once in ten sorts of 2^28 keys).  60 repetitions
+    per pass structure: equal to the library sort of numpy the first time, bit-identical afterwards."""
+    n = (1 << logn) + 12345
+    keys, vals = make(kind, n, seed=logn)
+    src_k, src_v = dev(keys), dev(vals)
+    for o in (RPP[1], RPP[2], RPP[3]):
+        ref = None
+        for rep in range(60):
+            dk, dv = src_k.clone(), None if src_v is None else src_v.clone()
+            bcf.sort(dk, dv, opts=o)
+            if ref is None:
+                ref = (dk, dv)
+                order = np.lexsort((vals, keys)) if vals is not None else np.argsort(keys, kind="stable")
+                assert np.array_equal(host(dk, keys), keys[order])
+                if vals is not None:
+                    assert np.array_equal(host(dv, vals), vals[order])
+            else:
+                assert torch.equal(dk, ref[0]) and (dv is None or torch.equal(dv, ref[1])), (kind, o, rep)
+
