@@ -141,7 +141,9 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
  *   merge_impl      BCF_MERGE_IMPL_AUTO, or BCF_MERGE_IMPL_GENERIC = one warp per page with loads from global
  *                   memory (merge_kernel) even where the TMA-fed pipeline applies; BCF_MERGE_IMPL_BARRIER4 =
  *                   four-run passes (rounds_per_pass = 2) always with the kernel that separates its two levels
- *                   by CTA barriers (bcf_merge4.cuh) instead of the task-stream kernel (bcf_merge4s.cuh).
+ *                   by CTA barriers (bcf_merge4.cuh) instead of the task-stream kernel (bcf_merge4s.cuh);
+ *                   BCF_MERGE_IMPL_PARTITION_LAUNCH = every round's split points from a partition launch, even
+ *                   where the merge kernel's CTAs would find their own (rounds with at most 8 shares per CTA).
  *   partition_warp_search_max
  *                   largest number of share boundaries of a round searched with 32 lanes per boundary
  *                   (latency-bound case); above it one thread per boundary.  < 0 = default (4096).
@@ -151,7 +153,7 @@ bcf_status bcf_sort_long_tiles(void *d_keys, void *d_vals, size_t num_long_tiles
  *                   (dependent launches: measured faster at every size, 27 % at 2^20 keys, 1 % at 2^28).
  */
 typedef enum { BCF_BASE_SHEARSORT = 0, BCF_BASE_TILE_MERGESORT = 1, BCF_BASE_LONG_TILES = 2, BCF_BASE_AUTO = 3 } bcf_base_case;
-typedef enum { BCF_MERGE_IMPL_AUTO = 0, BCF_MERGE_IMPL_GENERIC = 1, BCF_MERGE_IMPL_BARRIER4 = 2 } bcf_merge_impl;
+typedef enum { BCF_MERGE_IMPL_AUTO = 0, BCF_MERGE_IMPL_GENERIC = 1, BCF_MERGE_IMPL_BARRIER4 = 2, BCF_MERGE_IMPL_PARTITION_LAUNCH = 3 } bcf_merge_impl;
 typedef enum { BCF_LAUNCH_AUTO = 0, BCF_LAUNCH_PLAIN = 1, BCF_LAUNCH_PDL = 2 } bcf_launch_mode;
 typedef struct bcf_options {
     uint32_t struct_size;

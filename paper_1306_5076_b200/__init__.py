@@ -39,6 +39,7 @@ from .binding import (  # noqa: F401
     MERGE_IMPL_AUTO,
     MERGE_IMPL_GENERIC,
     MERGE_IMPL_BARRIER4,
+    MERGE_IMPL_PARTITION_LAUNCH,
     LAUNCH_AUTO,
     LAUNCH_PLAIN,
     LAUNCH_PDL,

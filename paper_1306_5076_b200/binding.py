@@ -17,7 +17,7 @@ KERNEL_IDS = ("tile_sort", "tile_mergesort", "long_tile_2", "long_tile_4", "long
               "partition_share_1", "partition_share_32", "merge_pipe", "partition4", "merge4_pipe", "merge_pagewise",
               "merge_pieces", "merge4_stream")
 BASE_SHEARSORT, BASE_TILE_MERGESORT, BASE_LONG_TILES, BASE_AUTO = 0, 1, 2, 3
-MERGE_IMPL_AUTO, MERGE_IMPL_GENERIC, MERGE_IMPL_BARRIER4 = 0, 1, 2
+MERGE_IMPL_AUTO, MERGE_IMPL_GENERIC, MERGE_IMPL_BARRIER4, MERGE_IMPL_PARTITION_LAUNCH = 0, 1, 2, 3
 LAUNCH_AUTO, LAUNCH_PLAIN, LAUNCH_PDL = 0, 1, 2
 
 

@@ -80,12 +80,13 @@ bool resolve_options(const bcf_options *o, Opt *r)
     if (o->struct_size < sizeof(bcf_options)) return false;
     if (o->base_case < BCF_BASE_SHEARSORT || o->base_case > BCF_BASE_AUTO) return false;
     if (o->rounds_per_pass < 0 || o->rounds_per_pass > 2) return false;
-    if (o->merge_impl < BCF_MERGE_IMPL_AUTO || o->merge_impl > BCF_MERGE_IMPL_BARRIER4) return false;
+    if (o->merge_impl < BCF_MERGE_IMPL_AUTO || o->merge_impl > BCF_MERGE_IMPL_PARTITION_LAUNCH) return false;
     if (o->launch_mode < BCF_LAUNCH_AUTO || o->launch_mode > BCF_LAUNCH_PDL) return false;
     r->base_case = o->base_case;
     if (o->rounds_per_pass) r->rounds_per_pass = o->rounds_per_pass;
     r->generic_merge = o->merge_impl == BCF_MERGE_IMPL_GENERIC;
     r->merge4_barrier = o->merge_impl == BCF_MERGE_IMPL_BARRIER4;
+    r->no_self_partition = o->merge_impl == BCF_MERGE_IMPL_PARTITION_LAUNCH;
     if (o->partition_warp_search_max >= 0) r->warp_search_max = static_cast<unsigned long long>(o->partition_warp_search_max);
     r->launch_mode = o->launch_mode;
     return true;

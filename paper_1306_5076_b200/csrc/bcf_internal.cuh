@@ -99,6 +99,7 @@ struct Opt {
     int base_case = BCF_BASE_AUTO;
     int rounds_per_pass = 1;             // resolved: 1 or 2
     bool generic_merge = false;
+    bool no_self_partition = false;      // always a partition launch, even where the merge kernel could find its own split points
     bool merge4_barrier = false;         // four-run passes with the barrier kernel even where the task-stream kernel applies
     unsigned long long warp_search_max = 4096;
     int launch_mode = BCF_LAUNCH_AUTO;

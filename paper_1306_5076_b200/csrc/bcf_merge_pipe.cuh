@@ -100,7 +100,10 @@ struct Cfg {
     static constexpr size_t scratch_off = STAGES * stage_bytes;
     static constexpr size_t meta_off = scratch_off + size_t(NWC) * TILE * 4;
     static constexpr size_t bar_off = meta_off + STAGES * sizeof(ShareMeta);
-    static constexpr size_t total = bar_off + 2 * STAGES * 8;
+    // split points a CTA works out for itself (small launches, SELF_MAX shares per CTA at most: merge_pipe_kernel)
+    static constexpr int SELF_MAX = 8;
+    static constexpr size_t self_off = bar_off + 2 * STAGES * 8;
+    static constexpr size_t total = self_off + 2 * SELF_MAX * 4;
     static_assert(total + 1024 <= 227 * 1024, "stage buffers + scratch planes exceed the SM's shared memory");
     // 227 KiB of shared memory per SM, 1 KiB per CTA reserved by the system
     static constexpr int ctas_per_sm = (2 * (total + 1024) <= 227 * 1024) ? 2 : 1;
@@ -212,10 +215,35 @@ __device__ __forceinline__ int corank_smem(const unsigned char *kreg, const unsi
 // bandwidth-bound and the plain binary search (G = 1) is faster (measured).
 // Only launched for rounds with 2 L > SH.
 constexpr int PART_THREADS = 128;
-#ifndef BCF_PART_PROBES
-#define BCF_PART_PROBES 2
-#endif
-constexpr int PART_PROBES = BCF_PART_PROBES;
+
+// Co-rank of share boundary s (output diagonal `share` * s of the round, inside its pair) by a 32-ary search of the
+// calling warp: lane j probes i = lo + j * step, one ballot narrows the range 32-fold.  Same result in every lane.
+template <class E>
+__device__ __forceinline__ unsigned long long corank_global_warp(const void *__restrict__ kin, const uint32_t *__restrict__ vin,
+                                                                 const unsigned long long n, const unsigned long long L,
+                                                                 const unsigned long long out0, const int lane)
+{
+    const unsigned long long a0 = out0 / (2 * L) * (2 * L);
+    if (a0 >= n) return 0ull;
+    const unsigned long long alen = min(L, n - a0);
+    const unsigned long long b0 = a0 + alen;
+    const unsigned long long blen = min(L, n - b0);
+    const unsigned long long d = min(out0 - a0, alen + blen);
+    unsigned long long lo = d > blen ? d - blen : 0ull;
+    unsigned long long hi = min(d, alen);
+    while (lo < hi) {
+        const unsigned long long step = (hi - lo + 31) / 32;
+        const unsigned long long mid = lo + lane * step;
+        bool le = false;
+        if (mid < hi) le = elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid));
+        const unsigned long long c = __popc(__ballot_sync(0xFFFFFFFFu, le));
+        const unsigned long long nlo = c ? lo + (c - 1) * step + 1 : lo;
+        hi = min(hi, lo + c * step);
+        lo = nlo;
+    }
+    return lo;
+}
+
 template <class E, int G>
 __global__ void __launch_bounds__(PART_THREADS)
 partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
@@ -237,23 +265,13 @@ partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict_
     unsigned long long lo = d > blen ? d - blen : 0ull;
     unsigned long long hi = min(d, alen);
     if constexpr (G == 1) {
-        // one thread per boundary, PART_PROBES probes per round: the probes of a round are independent loads, so a
-        // round costs one memory latency and narrows the range PART_PROBES-fold (14 dependent rounds instead of the
-        // 27 of a binary search for a pair of 2^27-element runs; the launch is latency-bound)
+        // (several independent probes per round -- a 4-ary or 8-ary search in one thread -- shorten the dependent
+        // chain and were measured slower, 0.034 -> 0.038 / 0.051 ms: with many boundaries the launch is bound by the
+        // number of random probes into DRAM)
         while (lo < hi) {
-            const unsigned long long step = (hi - lo + PART_PROBES - 1) / PART_PROBES;
-            bool le[PART_PROBES];
-#pragma unroll
-            for (int q = 0; q < PART_PROBES; ++q) {
-                const unsigned long long mid = lo + q * step;
-                le[q] = mid < hi && elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid));
-            }
-            unsigned long long c = 0;      // the predicate is monotone: the probes that hold are a prefix
-#pragma unroll
-            for (int q = 0; q < PART_PROBES; ++q) c += le[q] ? 1u : 0u;
-            const unsigned long long nlo = c ? lo + (c - 1) * step + 1 : lo;
-            hi = min(hi, lo + c * step);
-            lo = nlo;
+            const unsigned long long mid = (lo + hi) >> 1;
+            if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
+            else hi = mid;
         }
     } else {
         while (lo < hi) {
@@ -407,7 +425,7 @@ template <class E>
 __global__ void __maxnreg__(Cfg<E>::max_regs)
 merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vin, void *__restrict__ kout,
                   uint32_t *__restrict__ vout, const uint32_t *__restrict__ splits, const unsigned long long n,
-                  const unsigned long long L, const unsigned long long num_shares)
+                  const unsigned long long L, const unsigned long long num_shares, const int self_part)
 {
     pdl_entry();
     using C = Cfg<E>;
@@ -430,6 +448,20 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
             mbar_init(&empty[s], C::PAGES);      // one arrival per page of the share
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // self_part: the launch is small (every CTA has at most SELF_MAX shares) and no partition launch preceded it.
+    // The warps of the CTA work out the split points of the CTA's own share boundaries first -- boundary q = 2 i + e
+    // is the start (e = 0) or the end (e = 1) of the CTA's i-th share -- one 32-ary search per warp at a time.  This
+    // removes one launch per round where launches are what a round costs (2^24 keys and below).
+    uint32_t *self_splits = reinterpret_cast<uint32_t *>(smem_raw + C::self_off);
+    if (self_part) {
+        const unsigned int mine =
+            blockIdx.x < num_shares ? static_cast<unsigned int>((num_shares - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0u;
+        for (unsigned int q = warp; q < 2 * mine; q += NW + 1) {
+            const unsigned long long sb = blockIdx.x + static_cast<unsigned long long>(q >> 1) * gridDim.x + (q & 1u);
+            const unsigned long long c = corank_global_warp<E>(kin_, vin, n, L, sb * SH, lane);
+            if (lane == 0) self_splits[q] = static_cast<uint32_t>(c);
+        }
     }
     __syncthreads();
 
@@ -472,8 +504,8 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
                 const unsigned long long b0 = a0 + alen;
                 const unsigned long long blen = min(L, n - b0);
                 const unsigned long long D0 = out0 - a0, D1 = D0 + cnt;
-                const unsigned long long I0 = splits[s];
-                const unsigned long long I1 = (D1 >= alen + blen) ? alen : splits[s + 1];
+                const unsigned long long I0 = self_part ? self_splits[2 * it] : splits[s];
+                const unsigned long long I1 = (D1 >= alen + blen) ? alen : (self_part ? self_splits[2 * it + 1] : splits[s + 1]);
                 const unsigned long long ga = a0 + I0, gb = b0 + (D0 - I0);
                 const int la = static_cast<int>(I1 - I0), lb = cnt - la;
                 unsigned long long ksa, kea, ksb, keb, vsa = 0, vea = 0, vsb = 0, veb = 0;

@@ -33,16 +33,23 @@ bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin
     if (shares == 0) return BCF_OK;
     bcf_status st = ensure_dyn_smem<pipe::merge_pipe_kernel<E>>(c.dev, C::total);
     if (st != BCF_OK) return st;
-    if (2 * run_len > (size_t)C::SH) {
-        st = launch_partition_share<E>(c, kin, vin, splits, n, run_len, 0);
-        if (st != BCF_OK) return st;
-    }
-    LaunchTimer t(BCF_KERNEL_MERGE, c.s);
     const unsigned long long cap = static_cast<unsigned long long>(C::ctas_per_sm) * c.dev.num_sms;
     const unsigned blocks = static_cast<unsigned>(shares < cap ? shares : cap);
+    // shares that cut through the runs need split points: from a partition launch, or -- small launches -- worked
+    // out by the merge kernel's own CTAs (merge_pipe_kernel, self_part)
+    int self_part = 0;
+    if (2 * run_len > (size_t)C::SH) {
+        if ((shares + blocks - 1) / blocks <= (unsigned long long)C::SELF_MAX && !c.opt.no_self_partition) {
+            self_part = 1;
+        } else {
+            st = launch_partition_share<E>(c, kin, vin, splits, n, run_len, 0);
+            if (st != BCF_OK) return st;
+        }
+    }
+    LaunchTimer t(BCF_KERNEL_MERGE, c.s);
     return launch(c, pipe::merge_pipe_kernel<E>, blocks, C::THREADS, C::total, kin, vin, kout, vout,
                   static_cast<const uint32_t *>(splits), static_cast<unsigned long long>(n),
-                  static_cast<unsigned long long>(run_len), shares);
+                  static_cast<unsigned long long>(run_len), shares, self_part);
 }
 
 template <class E>

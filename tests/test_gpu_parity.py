@@ -21,15 +21,17 @@ def bcf():
 
 
 # bcf_options of the pass structures of the merging phase
-RPP = {1: {"rounds_per_pass": 1}, 2: {"rounds_per_pass": 2}, 3: {"rounds_per_pass": 2, "merge_impl": 2}}
+RPP = {1: {"rounds_per_pass": 1}, 2: {"rounds_per_pass": 2}, 3: {"rounds_per_pass": 2, "merge_impl": 2},
+       4: {"rounds_per_pass": 1, "merge_impl": 3}}
 
 
-@pytest.fixture(params=[1, 2, 3], ids=["1round", "2rounds", "2rounds-barrier"])
+@pytest.fixture(params=[1, 2, 3, 4], ids=["1round", "2rounds", "2rounds-barrier", "1round-partition-launch"])
 def rpp(request):
     """The pass structures of the merging phase, passed per call in bcf_options: one round per pass
     (Lemma 2), two rounds per pass (four-run kernels: the task-stream kernel where it applies), and
-    two rounds per pass with the barrier version of the four-run kernel everywhere; the result must be the same
-    unique sorted output."""
+    two rounds per pass with the barrier version of the four-run kernel everywhere, and one round per pass with a
+    partition launch for every round (small rounds otherwise find their split points inside the merge kernel); the
+    result must be the same unique sorted output."""
     return request.param
 
 
