@@ -652,6 +652,11 @@ def main():
         dt = oracle_run(args.workload, keys, vals, run_len)
         cpu = {"value": sn / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "host_cores_total": os.cpu_count(), "sample": sample + ", once"}
+        if op == "sort" and vals is None:
+            # context only: a textbook library sort on the same sample (numpy's default sort, one thread)
+            t0 = time.perf_counter()
+            np.sort(keys)
+            cpu["textbook_sort"] = {"what": "numpy.sort on the same sample, 1 thread", "value": sn / (time.perf_counter() - t0), "unit": UNIT}
     summary = None
     kv = None
     if rank == 0 and world == 1 and not args.no_side and args.workload == "cfg4a" and not args.log2n:

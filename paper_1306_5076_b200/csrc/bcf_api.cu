@@ -194,6 +194,7 @@ struct Workspace {
     void *keys;
     uint32_t *vals;
     uint32_t *splits;
+    PageSamples samples;     // page heads / tails between merge rounds (bcf_internal.cuh)
     size_t bytes;
 };
 
@@ -209,6 +210,17 @@ Workspace carve(void *base, size_t n, bcf_key_t kt, bcf_val_t vt, bool with_data
     if (with_data && vt == BCF_VAL_U32) off += align_up(n * 4, 256);
     w.splits = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
     off += align_up((shares + 1) * 4 + 64, 256);   // + room for the uint4 entries of a four-run pass
+#ifndef BCF_NO_PAGE_SAMPLES                          // A/B only
+    if (shares) {                                  // two samples per page of 1024 elements
+        const size_t pages = n / TILE + 1;
+        w.samples.keys = b ? b + off : nullptr;
+        off += align_up(2 * pages * key_bytes(kt), 256);
+        if (vt == BCF_VAL_U32) {
+            w.samples.vals = reinterpret_cast<uint32_t *>(b ? b + off : nullptr);
+            off += align_up(2 * pages * 4, 256);
+        }
+    }
+#endif
     w.bytes = off;
     return w;
 }
@@ -242,8 +254,9 @@ int count_passes(size_t n, size_t run_len, size_t stop_len, bcf_key_t kt, bcf_va
 // Pass i writes to dst[i]; each pass is one read + one write of all n elements.
 template <class E>
 bcf_status merge_rounds(const Call &c, const void *k0, const uint32_t *v0, void *ka, uint32_t *va, void *kb, uint32_t *vb,
-                        bool first_to_a, size_t n, size_t run_len, size_t stop_len, uint32_t *splits)
+                        bool first_to_a, size_t n, size_t run_len, size_t stop_len, uint32_t *splits, const PageSamples &samples)
 {
+    bool samples_valid = false;          // `samples` describes ksrc (the previous pass was a pipelined two-run round)
     const void *ksrc = k0;
     const uint32_t *vsrc = v0;
     bool to_a = first_to_a;
@@ -256,9 +269,12 @@ bcf_status merge_rounds(const Call &c, const void *k0, const uint32_t *v0, void 
         bcf_status st;
         if (ways[i] == 4) {
             st = launch_merge4<E>(c, ksrc, vsrc, kd, vd, splits, n, l);
+            samples_valid = false;
         } else if (pipe_eligible(l, c.opt)) {
-            st = launch_merge_pipe<E>(c, ksrc, vsrc, kd, vd, splits, n, l);
+            st = launch_merge_pipe<E>(c, ksrc, vsrc, kd, vd, splits, n, l, samples_valid ? samples : PageSamples(), samples);
+            samples_valid = samples.keys != nullptr && E::NP < 3;      // the three-plane kernel writes none (bcf_merge_pipe.cuh)
         } else {
+            samples_valid = false;
             const PassGeom g = pass_geom(n, l);
             st = launch_partition<E>(c, ksrc, vsrc, splits, g);
             if (st != BCF_OK) return st;
@@ -339,7 +355,7 @@ bcf_status merge_runs_common(bool pagewise, const void *d_keys_in, const void *d
     } else {
         BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, d_keys_in, static_cast<const uint32_t *>(d_vals_in), d_keys_out,
                                                   static_cast<uint32_t *>(d_vals_out), w.keys, w.vals, first_to_out, n,
-                                                  run_len, n, w.splits));
+                                                  run_len, n, w.splits, w.samples));
     }
     return st;
 }
@@ -377,7 +393,7 @@ bcf_status sort_phases(const Call &c, void *d_keys, void *d_vals, size_t n, size
     if (st != BCF_OK || passes == 0) return st;
     // pass 1 writes to the buffer the base case did not write.
     BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, base_run,
-                                              stop_len, w.splits));
+                                              stop_len, w.splits, w.samples));
     return st;
 }
 
@@ -893,7 +909,7 @@ bcf_status bcf_debug_merge_round_isolated(const void *d_keys_in, void *d_keys_ou
     if (st != BCF_OK) return st;
     ProfileGroup profile_group(stream);
     uint32_t *splits = static_cast<uint32_t *>(d_workspace);
-    st = launch_partition_share<E_U32>(c, d_keys_in, nullptr, splits, n, run_len, isolated_share());
+    st = launch_partition_share<E_U32>(c, d_keys_in, nullptr, splits, n, run_len, isolated_share(), nullptr, nullptr);
     if (st != BCF_OK) return st;
     return launch_isolated_merge_round(c, static_cast<const uint32_t *>(d_keys_in), static_cast<uint32_t *>(d_keys_out), splits, n,
                                        run_len, exclusive);

@@ -177,13 +177,21 @@ bcf_status launch_pagewise(const Call &c, const void *kin, const uint32_t *vin, 
 template <class E>
 bool kernel_desc_merge(int id, KernelDesc *k);
 // bcf_tu_pipe.cu
+// First and last element of every full page (1024 elements) of an array of sorted runs, written by the merge round
+// that produced the array and read by the partition of the next round: keys[2 p], keys[2 p + 1] (and vals) = head
+// and tail of page p.  keys == nullptr: none (not asked for / not valid).
+struct PageSamples {
+    void *keys = nullptr;
+    uint32_t *vals = nullptr;
+};
 // share = 0: the share size of the production merge kernel for E
 template <class E>
 bcf_status launch_partition_share(const Call &c, const void *kin, const uint32_t *vin, uint32_t *splits, size_t n, size_t run_len,
-                                  size_t share);
+                                  size_t share, const void *samp_k, const uint32_t *samp_v);
+// `in`: samples of kin (or none), `out`: where to write the samples of kout (or none)
 template <class E>
 bcf_status launch_merge_pipe(const Call &c, const void *kin, const uint32_t *vin, void *kout, uint32_t *vout, uint32_t *splits,
-                             size_t n, size_t run_len);
+                             size_t n, size_t run_len, const PageSamples &in, const PageSamples &out);
 template <class E>
 bool kernel_desc_pipe(int id, KernelDesc *k);
 // bcf_tu_merge4.cu

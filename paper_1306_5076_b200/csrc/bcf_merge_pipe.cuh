@@ -248,7 +248,7 @@ template <class E, int G>
 __global__ void __launch_bounds__(PART_THREADS)
 partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict__ vin, uint32_t *__restrict__ splits,
                        const unsigned long long n, const unsigned long long L, const unsigned long long num_shares,
-                       const unsigned long long share)
+                       const unsigned long long share, const void *__restrict__ samp_k, const uint32_t *__restrict__ samp_v)
 {
     pdl_entry();
     const int j = threadIdx.x % G;                       // lane inside the group
@@ -265,9 +265,28 @@ partition_share_kernel(const void *__restrict__ kin, const uint32_t *__restrict_
     unsigned long long lo = d > blen ? d - blen : 0ull;
     unsigned long long hi = min(d, alen);
     if constexpr (G == 1) {
-        // (several independent probes per round -- a 4-ary or 8-ary search in one thread -- shorten the dependent
-        // chain and were measured slower, 0.034 -> 0.038 / 0.051 ms: with many boundaries the launch is bound by the
-        // number of random probes into DRAM)
+        // One thread per boundary, binary search.  ncu (profiles/r2_partition_full.md): 19 us for 16385 boundaries
+        // of a pair of 2^27-key runs, 49 MB read from DRAM, every unit idle -- the ~54 probes of a boundary are
+        // scattered over a 1 GiB array, each a DRAM (and TLB) miss, and several probes per round make it SLOWER
+        // (4 / 8 / 16 independent, clamped probes per round: 0.027 / 0.037 / 0.054 ms per launch): the launch is
+        // bound by the number of scattered probes.  So the probes are made local instead.  The merge kernel that
+        // wrote this round's input also wrote the first and the last element of each of its output pages (1024
+        // elements) to a small array (`samp`, 2 MB for 2^28 keys).  Because a share boundary is a multiple of the
+        // page size, the predicate at i = 1024 k needs exactly a page head of A and a page tail of B: the first 17
+        // of the 27 steps run on the samples, the last 10 inside one page of A and one of B.
+        if (samp_k != nullptr && alen == L && lo < hi) {
+            const unsigned long long pa = a0 / TILE;                   // page of A[0]
+            const unsigned long long pb = (b0 + d) / TILE;             // B[d - 1 - 1024 k] = tail of page pb - k - 1
+            const unsigned long long k0 = (lo + TILE - 1) / TILE;
+            unsigned long long klo = k0, khi = (hi + TILE - 1) / TILE;  // smallest k in [klo, khi] with NOT P(1024 k)
+            while (klo < khi) {
+                const unsigned long long km = (klo + khi) >> 1;
+                if (elem_le_global<E>(samp_k, samp_v, 2 * (pa + km), 2 * (pb - km - 1) + 1)) klo = km + 1;
+                else khi = km;
+            }
+            if (klo > k0) lo = max(lo, (klo - 1) * TILE + 1);
+            hi = min(hi, klo * TILE);
+        }
         while (lo < hi) {
             const unsigned long long mid = (lo + hi) >> 1;
             if (elem_le_global<E>(kin, vin, a0 + mid, b0 + (d - 1 - mid))) lo = mid + 1;
@@ -344,12 +363,22 @@ __device__ __forceinline__ void load_columns(uint32_t (&v)[E::NP][32], const int
 // element go through it one after the other.  Same access patterns, same conflict-freedom.
 template <class E>
 __device__ __forceinline__ void store_rows_seq(uint32_t *scratch, void *keys, uint32_t *vals, const size_t base,
-                                               const int cnt, const bool full, const int lane, uint32_t (&v)[E::NP][32])
+                                               const int cnt, const bool full, const int lane, uint32_t (&v)[E::NP][32],
+                                               void *samp_k = nullptr, uint32_t *samp_v = nullptr)
 {
+    // samp_k / samp_v (optional): first and last element of a FULL page go to entries 2 p, 2 p + 1 (p = base / 1024)
+    // of the sample arrays -- read by lane 0 from the scratch plane while the plane holds them (words of logical
+    // (row 0, column 0) and (row 31, column 31)), so that no register of the page stays live for it.
+    // Not for three-plane elements: their kernel sits at its register cap and any addition costs it 3-9 % per round
+    // (measured), more than the partition launch gains; their partition searches the arrays themselves.
+    const size_t se = 2 * (base / TILE);
+    const bool sample = E::NP < 3 && samp_k != nullptr && lane == 0;
     if (full) {
         if constexpr (E::KEY_WORDS == 1) {
             row_store(scratch, v[0], lane);
             __syncwarp();
+            if (sample)
+                *reinterpret_cast<uint2 *>(static_cast<uint32_t *>(samp_k) + se) = make_uint2(scratch[elem_word(0, 0)], scratch[elem_word(31, 31)]);
             uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint32_t *>(keys) + base);
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
@@ -359,6 +388,8 @@ __device__ __forceinline__ void store_rows_seq(uint32_t *scratch, void *keys, ui
         } else {
             row_store(scratch, v[0], lane);
             __syncwarp();
+            uint32_t sh0 = 0, sh1 = 0;
+            if (sample) { sh0 = scratch[elem_word(0, 0)]; sh1 = scratch[elem_word(31, 31)]; }
 #pragma unroll
             for (int m = 0; m < 16; ++m) {     // this lane's high words of keys 64 m + 2 lane, + 1
                 const int w = elem_word(2 * m + (lane >> 4), 2 * (lane & 15));
@@ -368,6 +399,9 @@ __device__ __forceinline__ void store_rows_seq(uint32_t *scratch, void *keys, ui
             __syncwarp();
             row_store(scratch, v[1], lane);
             __syncwarp();
+            if (sample)
+                *reinterpret_cast<uint4 *>(static_cast<uint64_t *>(samp_k) + se) =
+                    make_uint4(scratch[elem_word(0, 0)], sh0, scratch[elem_word(31, 31)], sh1);
             uint4 *pk = reinterpret_cast<uint4 *>(static_cast<uint64_t *>(keys) + base);
 #pragma unroll
             for (int m = 0; m < 16; ++m) {
@@ -380,6 +414,7 @@ __device__ __forceinline__ void store_rows_seq(uint32_t *scratch, void *keys, ui
             __syncwarp();
             row_store(scratch, v[E::KEY_WORDS], lane);
             __syncwarp();
+            if (sample) *reinterpret_cast<uint2 *>(samp_v + se) = make_uint2(scratch[elem_word(0, 0)], scratch[elem_word(31, 31)]);
             uint4 *pv = reinterpret_cast<uint4 *>(vals + base);
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
@@ -425,7 +460,8 @@ template <class E>
 __global__ void __maxnreg__(Cfg<E>::max_regs)
 merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vin, void *__restrict__ kout,
                   uint32_t *__restrict__ vout, const uint32_t *__restrict__ splits, const unsigned long long n,
-                  const unsigned long long L, const unsigned long long num_shares, const int self_part)
+                  const unsigned long long L, const unsigned long long num_shares, const int self_part,
+                  void *__restrict__ samp_k, uint32_t *__restrict__ samp_v)
 {
     pdl_entry();
     using C = Cfg<E>;
@@ -617,7 +653,9 @@ merge_pipe_kernel(const void *__restrict__ kin_, const uint32_t *__restrict__ vi
         }
         line_bitonic_merge<E::NP>(v);            // row pass
         const int cnt = d1 - d0;
-        store_rows_seq<E>(scratch, kout, vout, s * SH + tile_off, cnt, cnt == TILE, lane, v);
+        // (full pages also leave their first and last element in `samp` for the partition of the next round)
+        if constexpr (E::NP < 3) store_rows_seq<E>(scratch, kout, vout, s * SH + tile_off, cnt, cnt == TILE, lane, v, samp_k, samp_v);
+        else store_rows_seq<E>(scratch, kout, vout, s * SH + tile_off, cnt, cnt == TILE, lane, v);
     }
 }
 
