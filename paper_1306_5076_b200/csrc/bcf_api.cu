@@ -370,32 +370,91 @@ void resolve_base_case(const Opt &o, bcf_key_t kt, bcf_val_t vt, int *bc, size_t
 }
 
 // Base case + merge passes until runs of at least stop_len (stop_len >= n: the whole sort), in place: the
-// result is in d_keys / d_vals.  Validation is the caller's.
+// result is in d_keys / d_vals.  Validation is the caller's.  The two phases are separate functions so that
+// bcf_sort_host can run the base case chunk by chunk under the host-to-device copy.
+struct SortPlan {
+    int bc;                  // base case network
+    size_t base_run;         // length of the runs it leaves
+    int passes;              // merge passes after it
+    Workspace w;
+    void *k0;                // where the base case writes: with an odd number of merge passes the workspace, so that the
+    uint32_t *v0;            // last pass lands in the caller's buffer without an extra copy
+    bool base_to_ws;
+};
+
+SortPlan sort_plan(const Call &c, void *d_keys, void *d_vals, size_t n, size_t stop_len, bcf_key_t kt, bcf_val_t vt, void *d_workspace)
+{
+    SortPlan p;
+    resolve_base_case(c.opt, kt, vt, &p.bc, &p.base_run);
+    p.passes = n > p.base_run ? count_passes(n, p.base_run, stop_len, kt, vt, c.opt) : 0;
+    p.w = carve(d_workspace, n, kt, vt, n > TILE, n > TILE ? max_shares(n, TILE) : 0);
+    p.base_to_ws = (p.passes % 2 == 1);
+    p.k0 = p.base_to_ws ? p.w.keys : d_keys;
+    p.v0 = p.base_to_ws ? p.w.vals : static_cast<uint32_t *>(d_vals);
+    return p;
+}
+
+// base case of elements [first, first + count) (first a multiple of the base run length)
+bcf_status sort_base_case(const Call &c, const SortPlan &p, void *d_keys, void *d_vals, size_t first, size_t count, bcf_key_t kt,
+                          bcf_val_t vt)
+{
+    const size_t kb = key_bytes(kt);
+    const void *kin = static_cast<const char *>(d_keys) + first * kb;
+    const uint32_t *vin = d_vals ? static_cast<const uint32_t *>(d_vals) + first : nullptr;
+    void *kout = static_cast<char *>(p.k0) + first * kb;
+    uint32_t *vout = p.v0 ? p.v0 + first : nullptr;
+    bcf_status st;
+    if (p.bc == BCF_BASE_LONG_TILES)
+        BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(c, kin, vin, kout, vout, count, BCF_LONG_TILE_H));
+    else
+        BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(c, kin, vin, kout, vout, count, p.bc));
+    return st;
+}
+
+bcf_status sort_merge_phase(const Call &c, const SortPlan &p, void *d_keys, void *d_vals, size_t n, size_t stop_len, bcf_key_t kt,
+                            bcf_val_t vt)
+{
+    if (p.passes == 0) return BCF_OK;
+    bcf_status st;
+    // pass 1 writes to the buffer the base case did not write.
+    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, p.k0, p.v0, d_keys, static_cast<uint32_t *>(d_vals), p.w.keys, p.w.vals,
+                                              /*first_to_a=*/p.base_to_ws, n, p.base_run, stop_len, p.w.splits, p.w.samples));
+    return st;
+}
+
 bcf_status sort_phases(const Call &c, void *d_keys, void *d_vals, size_t n, size_t stop_len, bcf_key_t kt, bcf_val_t vt,
                        void *d_workspace)
 {
-    int bc;
-    size_t base_run;
-    resolve_base_case(c.opt, kt, vt, &bc, &base_run);
-    const int passes = n > base_run ? count_passes(n, base_run, stop_len, kt, vt, c.opt) : 0;
-    const Workspace w = carve(d_workspace, n, kt, vt, n > TILE, n > TILE ? max_shares(n, TILE) : 0);
-    uint32_t *vals = static_cast<uint32_t *>(d_vals);
-    // With an odd number of merge passes the base case writes into the workspace, so that the
-    // last pass lands in the caller's buffer without an extra copy.
-    const bool base_to_ws = (passes % 2 == 1);
-    void *k0 = base_to_ws ? w.keys : d_keys;
-    uint32_t *v0 = base_to_ws ? w.vals : vals;
-    bcf_status st;
-    if (bc == BCF_BASE_LONG_TILES)
-        BCF_DISPATCH(kt, vt, st = launch_long_tile<E>(c, d_keys, vals, k0, v0, n, BCF_LONG_TILE_H));
-    else
-        BCF_DISPATCH(kt, vt, st = launch_tile_sort<E>(c, d_keys, vals, k0, v0, n, bc));
-    if (st != BCF_OK || passes == 0) return st;
-    // pass 1 writes to the buffer the base case did not write.
-    BCF_DISPATCH(kt, vt, st = merge_rounds<E>(c, k0, v0, d_keys, vals, w.keys, w.vals, /*first_to_a=*/base_to_ws, n, base_run,
-                                              stop_len, w.splits, w.samples));
-    return st;
+    const SortPlan p = sort_plan(c, d_keys, d_vals, n, stop_len, kt, vt, d_workspace);
+    const bcf_status st = sort_base_case(c, p, d_keys, d_vals, 0, n, kt, vt);
+    if (st != BCF_OK) return st;
+    return sort_merge_phase(c, p, d_keys, d_vals, n, stop_len, kt, vt);
 }
+
+// side stream + events of one bcf_sort_host call (created per call: tens of microseconds against tens of milliseconds of copies)
+struct HostOverlap {
+    static constexpr int CHUNKS = 8;
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev[CHUNKS + 1] = {};
+    cudaEvent_t done = nullptr;
+    bcf_status init()
+    {
+        BCF_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+        for (auto &e : ev) BCF_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        BCF_CUDA(cudaEventCreateWithFlags(&done, cudaEventDisableTiming));
+        return BCF_OK;
+    }
+    ~HostOverlap()
+    {
+        if (side) {
+            cudaStreamSynchronize(side);
+            cudaStreamDestroy(side);
+        }
+        for (auto &e : ev)
+            if (e) cudaEventDestroy(e);
+        if (done) cudaEventDestroy(done);
+    }
+};
 
 bcf_status validate_sort(const void *d_keys, const void *d_vals, size_t n, bcf_key_t kt, bcf_val_t vt, const void *d_workspace,
                          size_t workspace_bytes)
@@ -875,10 +934,49 @@ bcf_status bcf_sort_host_ex(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, 
     void *dk = base;
     void *dv = vb ? base + align_up(kb, 256) : nullptr;
     const size_t data = align_up(kb, 256) + (vb ? align_up(vb, 256) : 0);
-    BCF_CUDA(cudaMemcpyAsync(dk, h_keys, kb, cudaMemcpyHostToDevice, stream));
-    if (vb) BCF_CUDA(cudaMemcpyAsync(dv, h_vals, vb, cudaMemcpyHostToDevice, stream));
-    const bcf_status st = bcf_sort_ex(dk, dv, n, kt, vt, base + data, scratch_bytes - data, stream, options);
+    Call c;
+    c.s = stream;
+    if (!resolve_options(options, &c.opt)) return BCF_ERR_INVALID_ARG;
+    bcf_status st = current_device(&c.dev);
     if (st != BCF_OK) return st;
+    resolve_launch_mode(&c.opt, n);
+    if (n <= TILE) {
+        BCF_CUDA(cudaMemcpyAsync(dk, h_keys, kb, cudaMemcpyHostToDevice, stream));
+        if (vb) BCF_CUDA(cudaMemcpyAsync(dv, h_vals, vb, cudaMemcpyHostToDevice, stream));
+        st = bcf_sort_ex(dk, dv, n, kt, vt, base + data, scratch_bytes - data, stream, options);
+        if (st != BCF_OK) return st;
+    } else {
+        // The base case works on independent tiles, so it runs chunk by chunk on a second stream while the next
+        // chunk is still being copied: only the last chunk's base case is left on the critical path.  The merge
+        // rounds need all the data and follow on the caller's stream.
+        ProfileGroup profile_group(stream);
+        const SortPlan p = sort_plan(c, dk, dv, n, n, kt, vt, base + data);
+        HostOverlap ov;
+        if ((st = ov.init()) != BCF_OK) return st;
+        Call side = c;
+        side.s = ov.side;
+        const size_t unit = p.base_run;
+        const size_t chunk = (n / HostOverlap::CHUNKS + unit - 1) / unit * unit;
+        int i = 0;
+        for (size_t first = 0; first < n; first += chunk, ++i) {
+            const size_t count = n - first < chunk ? n - first : chunk;
+            BCF_CUDA(cudaMemcpyAsync(static_cast<char *>(dk) + first * key_bytes(kt), static_cast<const char *>(h_keys) + first * key_bytes(kt),
+                                     count * key_bytes(kt), cudaMemcpyHostToDevice, stream));
+            if (vb)
+                BCF_CUDA(cudaMemcpyAsync(static_cast<uint32_t *>(dv) + first, static_cast<const uint32_t *>(h_vals) + first, count * 4,
+                                         cudaMemcpyHostToDevice, stream));
+            BCF_CUDA(cudaEventRecord(ov.ev[i], stream));
+            BCF_CUDA(cudaStreamWaitEvent(ov.side, ov.ev[i], 0));
+            if ((st = sort_base_case(side, p, dk, dv, first, count, kt, vt)) != BCF_OK) return st;
+        }
+        BCF_CUDA(cudaEventRecord(ov.done, ov.side));
+        BCF_CUDA(cudaStreamWaitEvent(stream, ov.done, 0));
+        if ((st = sort_merge_phase(c, p, dk, dv, n, n, kt, vt)) != BCF_OK) return st;
+        BCF_CUDA(cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream));
+        if (vb) BCF_CUDA(cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream));
+        BCF_CUDA(cudaStreamSynchronize(stream));      // before `ov` (the side stream and its events) goes away
+        return BCF_OK;
+    }
     BCF_CUDA(cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream));
     if (vb) BCF_CUDA(cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream));
     BCF_CUDA(cudaStreamSynchronize(stream));
