@@ -46,7 +46,9 @@ extern "C" {
 
 #define BCF_W 32            /* warp size = number of 4-byte shared memory banks */
 #define BCF_TILE 1024       /* M = w*w elements per tile / page           */
-#define BCF_SHARE 8192      /* outputs of a merge pass one CTA takes at a time (8 pages)              */
+#define BCF_SHARE 8192      /* outputs per share of the four-run pass (bcf_merge_partition4) and of the
+                               isolation experiment: 8 pages.  The two-run merge kernel picks its own share
+                               size per element type (16 / 4 / 8 pages for 4- / 8- / 12-byte elements).       */
 
 /* A CUDA stream handle; identical to cudaStream_t / CUstream. */
 typedef struct CUstream_st *bcf_stream_t;

@@ -531,7 +531,7 @@ const char *bcf_status_string(bcf_status s)
     return "BCF_ERR_UNKNOWN";
 }
 
-const char *bcf_version(void) { return "bcf 0.2 (sm_100a)"; }
+const char *bcf_version(void) { return "bcf 0.3 (sm_100a)"; }
 
 bcf_status bcf_options_init(bcf_options *opt)
 {
