@@ -105,6 +105,70 @@ __device__ __forceinline__ void tile_bitonic_merge(uint32_t *planes, const int l
     line_bitonic_merge<E::NP, BCF_LT_FMA_MOD>(v);
 }
 
+// The LAST cross-tile stage of a round with the exchange doubling as the row -> column transpose of the tile merge
+// that follows: the warp writes its rows to the exchange set as before, and after the barrier thread c reads BOTH
+// tiles in the column layout -- its own position 32 k + c and the partner's (for the flip: position 1023 - p, i.e.
+// row 31 - k, column 31 - c; for a fixed k one row in a permuted order, 32 distinct banks) -- and keeps the smaller
+// or the larger element.  The result is the column registers the column pass needs, so the row_store + col_load of
+// tile_bitonic_merge (one of this kernel's shared-memory sweeps per element and round) is not needed.
+#ifndef BCF_LT_FUSED_TRANSPOSE
+#define BCF_LT_FUSED_TRANSPOSE 1
+#endif
+template <class E, bool FLIP, bool LOW>
+__device__ __forceinline__ void cross_stage_cols_keep(const uint32_t *own, const uint32_t *partner, const int lane,
+                                                      uint32_t (&v)[E::NP][32])
+{
+    constexpr int NP = E::NP;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        uint32_t a[NP], b[NP];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            a[p] = own[p * TILE + elem_word(k, lane)];
+            b[p] = partner[p * TILE + (FLIP ? elem_word(31 - k, 31 - lane) : elem_word(k, lane))];
+        }
+        if constexpr (NP == 1) {
+            v[0][k] = LOW ? min(a[0], b[0]) : max(a[0], b[0]);
+        } else {
+            bool gt = false, eq = true;      // mine > other, lexicographic over the planes
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                gt = gt || (eq && a[p] > b[p]);
+                eq = eq && a[p] == b[p];
+            }
+            const bool take = LOW ? gt : !(gt || eq);
+#pragma unroll
+            for (int p = 0; p < NP; ++p) v[p][k] = take ? b[p] : a[p];
+        }
+    }
+}
+
+template <class E, bool FLIP>
+__device__ __forceinline__ void cross_stage_to_cols(uint32_t *set, const int warp, const int partner, const bool low, const int lane,
+                                                    uint32_t (&v)[E::NP][32])
+{
+    uint32_t *mine = set + warp * (E::NP * TILE);
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) row_store(mine + p * TILE, v[p], lane);
+    __syncthreads();
+    const uint32_t *other = set + partner * (E::NP * TILE);
+    if (low) cross_stage_cols_keep<E, FLIP, true>(mine, other, lane, v);
+    else cross_stage_cols_keep<E, FLIP, false>(mine, other, lane, v);
+}
+
+// column pass + row pass on a tile that holds a bitonic sequence in COLUMN registers
+template <class E>
+__device__ __forceinline__ void tile_bitonic_merge_cols(uint32_t *planes, const int lane, uint32_t (&v)[E::NP][32])
+{
+    line_bitonic_merge<E::NP, BCF_LT_FMA_MOD>(v);
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) col_store<false>(planes + p * TILE, v[p], lane);
+    __syncwarp();
+#pragma unroll
+    for (int p = 0; p < E::NP; ++p) row_load(planes + p * TILE, v[p], lane);
+    line_bitonic_merge<E::NP, BCF_LT_FMA_MOD>(v);
+}
+
 template <class E, int H>
 struct LongTileCfg {
     static constexpr size_t set_words = size_t(H) * E::NP * TILE;
@@ -147,11 +211,24 @@ long_tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t
 #pragma unroll
         for (int B = 2; B <= H; B *= 2) {
             const int i = warp & (B - 1);
+#if BCF_LT_FUSED_TRANSPOSE
+            if (B == 2) {
+                cross_stage_to_cols<E, true>(smem + (stage++ & 1) * SET, warp, (warp - i) + (B - 1 - i), i < B / 2, lane, v);
+            } else {
+                cross_stage<E, true>(smem + (stage++ & 1) * SET, warp, (warp - i) + (B - 1 - i), i < B / 2, lane, v);
+#pragma unroll
+                for (int s = B / 4; s >= 2; s /= 2)
+                    cross_stage<E, false>(smem + (stage++ & 1) * SET, warp, warp ^ s, (warp & s) == 0, lane, v);
+                cross_stage_to_cols<E, false>(smem + (stage++ & 1) * SET, warp, warp ^ 1, (warp & 1) == 0, lane, v);
+            }
+            tile_bitonic_merge_cols<E>(slot + (stage & 1) * SET, lane, v);
+#else
             cross_stage<E, true>(smem + (stage++ & 1) * SET, warp, (warp - i) + (B - 1 - i), i < B / 2, lane, v);
 #pragma unroll
             for (int s = B / 4; s >= 1; s /= 2)
                 cross_stage<E, false>(smem + (stage++ & 1) * SET, warp, warp ^ s, (warp & s) == 0, lane, v);
             tile_bitonic_merge<E>(slot + (stage & 1) * SET, lane, v);
+#endif
         }
         // (storing the rows straight from the registers -- eight 16-byte stores per thread, 128 bytes apart across
         // the lanes -- would save this round trip through shared memory; measured slower, 1.71 -> 1.84 ms: the
