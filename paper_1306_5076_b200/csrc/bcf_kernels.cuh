@@ -286,6 +286,10 @@ tile_sort_kernel(const void *kin, const uint32_t *vin, void *kout, uint32_t *vou
 #ifndef BCF_TMS_FMA_MOD
 #define BCF_TMS_FMA_MOD 0     // min/max only: this kernel is not bound by the ALU pipe (A/B in DESIGN.md 5.6)
 #endif
+// (Level T = 1 with warp shuffles instead of shared memory -- the two rows of a block live in neighbouring threads, both
+// send register 31 - j and keep min / max with one predicated VIMNMX -- was built and measured in r2: 32 SHFL.BFLY in
+// place of four sweeps through shared memory gain 0.5 % on the long-tile kernel; a shuffle occupies the same data
+// path about as long as the wavefronts it replaces.  Not kept.)
 template <class E, int T, int FM = BCF_TMS_FMA_MOD>
 __device__ __forceinline__ void tile_merge_level(uint32_t *planes, const int lane, uint32_t (&v)[E::NP][32])
 {
