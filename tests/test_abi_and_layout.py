@@ -248,6 +248,9 @@ def test_argument_errors_are_reported_before_any_device_work():
     bad.base_case = 9
     assert L.bcf_sort_ex(p, None, 4096, 0, 0, p + 32768, 1 << 15, None, ctypes.byref(bad)) == INVALID
     bad = bcf.options()
+    bad.merge_impl = 4                                            # one past BCF_MERGE_IMPL_PARTITION_LAUNCH
+    assert L.bcf_sort_ex(p, None, 4096, 0, 0, p + 32768, 1 << 15, None, ctypes.byref(bad)) == INVALID
+    bad = bcf.options()
     bad.struct_size = 8
     assert L.bcf_merge_pass_count(1 << 20, 1024, 0, 0, ctypes.byref(bad)) == 0
     # BCFMergesort with buckets: P >= 2, t >= 1, workspace
