@@ -244,7 +244,7 @@ bcf_status bcf_find_buckets(const void *d_keys_in, size_t n, size_t run_len, int
  *               reproduce its Figure 1 (bank conflicts and run time grow with d).  Same result.
  *   d_out     : n uint32, may not overlap the inputs.
  *   d_workspace : >= bcf_colored_prefix_sums_workspace_bytes(n) bytes.
- * A colour >= num_colors is an unchecked precondition violation.
+ * A colour >= num_colors is counted as colour num_colors - 1 (it never indexes outside the caller's d sums).
  */
 typedef enum { BCF_SCAN_BANK_PER_THREAD = 0, BCF_SCAN_THREAD_MAJOR = 1 } bcf_scan_layout;
 size_t bcf_colored_prefix_sums_workspace_bytes(size_t n);

@@ -63,8 +63,8 @@ __device__ __forceinline__ void warp_pages(const unsigned long long n, const uns
 
 // this lane's chunk of a page: CH values and CH colours (missing elements: value 0, colour 0)
 __device__ __forceinline__ void load_chunk(const uint32_t *__restrict__ vals, const unsigned char *__restrict__ cols,
-                                           const unsigned long long base, const unsigned long long n, uint32_t (&v)[CH],
-                                           uint32_t (&c)[CH])
+                                           const unsigned long long base, const unsigned long long n, const int d,
+                                           uint32_t (&v)[CH], uint32_t (&c)[CH])
 {
     if (base + CH <= n) {
         const uint4 *pv = reinterpret_cast<const uint4 *>(vals + base);
@@ -88,6 +88,9 @@ __device__ __forceinline__ void load_chunk(const uint32_t *__restrict__ vals, co
             c[k] = in ? cols[base + k] : 0u;
         }
     }
+    // a colour byte >= d comes straight from the caller's data and would index another warp's sums: counted as d - 1
+#pragma unroll
+    for (int k = 0; k < CH; ++k) c[k] = min(c[k], static_cast<uint32_t>(d - 1));
 }
 
 // Phase 1: partial[w][c] = sum of the values of colour c in warp w's tile.
@@ -106,7 +109,7 @@ reduce_kernel(const uint32_t *__restrict__ vals, const unsigned char *__restrict
     for (int c = 0; c < d; ++c) s[slot<CF>(c, lane, d)] = 0;
     for (unsigned long long p = first; p < last; ++p) {
         uint32_t v[CH], c[CH];
-        load_chunk(vals, cols, p * PAGE + lane * CH, n, v, c);
+        load_chunk(vals, cols, p * PAGE + lane * CH, n, d, v, c);
 #pragma unroll
         for (int k = 0; k < CH; ++k) s[slot<CF>(c[k], lane, d)] += v[k];
     }
@@ -153,7 +156,7 @@ scan_kernel(const uint32_t *__restrict__ vals, const unsigned char *__restrict__
     for (unsigned long long p = first; p < last; ++p) {
         const unsigned long long base = p * PAGE + lane * CH;
         uint32_t v[CH], c[CH];
-        load_chunk(vals, cols, base, n, v, c);
+        load_chunk(vals, cols, base, n, d, v, c);
         for (int k = 0; k < d; ++k) s[slot<CF>(k, lane, d)] = 0;
         // running sums inside the chunk: one read-modify-write of this lane's own word per element
 #pragma unroll

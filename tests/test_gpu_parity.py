@@ -493,6 +493,17 @@ def test_colored_prefix_sums_match_oracle(bcf, layout, n, d):
     assert np.array_equal(host(out, vals), oracle.colored_prefix_sums(vals, cols, d))
 
 
+@pytest.mark.parametrize("layout", [0, 1], ids=["bank_per_thread", "thread_major"])
+def test_colored_prefix_sums_out_of_range_colour_is_clamped(bcf, layout):
+    """include/bcf.h: a colour byte >= num_colors counts as colour num_colors - 1 and never touches another warp's sums."""
+    n, d = 40000, 4
+    rng = np.random.default_rng(5)
+    vals = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(np.uint32)
+    cols = rng.integers(0, 256, size=n).astype(np.uint8)
+    out = bcf.colored_prefix_sums(dev(vals), torch.from_numpy(cols).cuda(), d, layout=layout)
+    assert np.array_equal(host(out, vals), oracle.colored_prefix_sums(vals, np.minimum(cols, d - 1).astype(np.uint8), d))
+
+
 # ---------------------------------------------------------------- bcf_sort_buckets / bcf_merge_pieces (SURVEY 8f item 2)
 
 
