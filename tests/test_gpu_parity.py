@@ -343,13 +343,18 @@ def test_sort_empty_is_noop(bcf):
     assert bcf.merge_runs(e, 4).numel() == 0
 
 
-def test_sort_host_roundtrip(bcf):
-    keys, vals = make("u64u32", 50000, seed=1)
-    hk = torch.from_numpy(keys.view(np.int64).copy()).pin_memory()
-    hv = torch.from_numpy(vals.view(np.int32).copy()).pin_memory()
-    bcf.sort_host(hk, hv)
-    wk, wv = oracle.sort_full(keys, vals)
-    assert np.array_equal(hk.numpy().view(np.uint64), wk) and np.array_equal(hv.numpy().view(np.uint32), wv)
+@pytest.mark.parametrize("kind,n", [("u64u32", 50000), ("u32", 700), ("u32", 1024), ("u32", 4 * 8192), ("u32", 4 * 8192 + 1),
+                                    ("u32", 1234567), ("u32u32", 300001), ("u64", 99999)])
+def test_sort_host_roundtrip(bcf, kind, n, rpp):
+    """bcf_sort_host copies the input in chunks and sorts the tiles of a chunk on a second stream while the next chunk is
+    copied (chunks are whole base-case runs; ragged last chunk, fewer elements than chunks, odd and even pass counts)."""
+    keys, vals = make(kind, n, seed=1)
+    signed = {np.dtype(np.uint32): np.int32, np.dtype(np.uint64): np.int64}[keys.dtype]
+    hk = torch.from_numpy(keys.view(signed).copy()).pin_memory()
+    hv = None if vals is None else torch.from_numpy(vals.view(np.int32).copy()).pin_memory()
+    bcf.sort_host(hk, hv, opts={**RPP[rpp]})
+    want = oracle.sort_full(keys, vals)
+    assert_same(hk.numpy().view(keys.dtype), None if hv is None else hv.numpy().view(np.uint32), want, vals)
 
 
 # ---------------------------------------------------------------- error behaviour (include/bcf.h)
