@@ -587,8 +587,9 @@ def main():
         # integer min/max issue at 64 lanes / clk / SM.
         sm_mhz = clocks.get("sm_max_mhz") or 1965.0
         # ALU-pipe instructions per comparator, from the SASS: u32 = VIMNMX min + max = 2; two planes = 2 subtract-with-
-        # borrow (IADD3 / IADD3.X into a predicate) + 4 SEL = 6; three planes = 3 + 6 = 9
-        ops = n * 11 * 191 / 32 * {"u32": 2, "u32+u32": 6, "u64": 6, "u64+u32": 9}[dtype]
+        # borrow (IADD3 / IADD3.X into a predicate) + 3 SEL = 5 (the fourth output is formed with 2 IMADs on the FMA
+        # pipe, BCF_CE2_FMA_PLANES = 1); three planes = 3 + 6 SEL = 9
+        ops = n * 11 * 191 / 32 * {"u32": 2, "u32+u32": 5, "u64": 5, "u64+u32": 9}[dtype]
         peak_ops = 148 * 64 * sm_mhz * 1e6
         ach = ops / (d_ms / d_cnt * 1e-3)
         roofline = {"kernel": "tile_sort_kernel (one launch = ShearSort of all tiles)", "bound": "alu",
