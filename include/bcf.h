@@ -18,7 +18,8 @@
  *    16-byte aligned (BCF_ERR_MISALIGNED otherwise).  d_vals must be NULL iff the value type is
  *    BCF_VAL_NONE.
  *  - OWNERSHIP: the caller owns every byte, including the workspace; the library never
- *    allocates or frees device memory.
+ *    allocates or frees device memory.  (One call, bcf_merge_round_static, takes no workspace: its
+ *    scratch is a fixed 256 KiB array inside the library's device image; see there.)
  *  - ASYNCHRONY: device entry points only enqueue work on `stream` and return; they never
  *    synchronise.  (bcf_sort_host is the exception, see there.)
  *  - ERRORS: status codes only; no exceptions, no exit().  n == 0 is BCF_OK and a no-op.
@@ -59,7 +60,9 @@ typedef enum {
     BCF_ERR_MISALIGNED = 2,          /* a device pointer is not 16-byte aligned                         */
     BCF_ERR_WORKSPACE_TOO_SMALL = 3, /* workspace_bytes < bcf_workspace_bytes(...)                      */
     BCF_ERR_UNSUPPORTED_DEVICE = 4,  /* current device is not compute capability 10.x                   */
-    BCF_ERR_CUDA = 5                 /* a CUDA runtime call or kernel launch failed                     */
+    BCF_ERR_CUDA = 5,                /* a CUDA runtime call or kernel launch failed                     */
+    BCF_ERR_TOO_LARGE = 6            /* bcf_merge_round_static only: the round needs more split points
+                                        than the library's built-in scratch array holds                 */
 } bcf_status;
 
 typedef enum { BCF_KEY_U32 = 0, BCF_KEY_U64 = 1 } bcf_key_t;
@@ -284,6 +287,52 @@ bcf_status bcf_merge_runs(const void *d_keys_in, const void *d_vals_in, void *d_
 bcf_status bcf_merge_runs_ex(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
                              size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt,
                              void *d_workspace, size_t workspace_bytes, bcf_stream_t stream, const bcf_options *opt);
+
+/*
+ * bcf_merge_round_static -- ONE merge round (section 3: adjacent runs merged in pairs) that needs
+ * no workspace and allocates nothing.
+ *
+ * Why it exists.  bcf_merge_runs wants a workspace, and a caller normally gets one from cudaMalloc.  Not every
+ * caller can: code that a host engine runs inside its execute step (an inference plugin, a framework operator)
+ * is often not allowed to allocate there; a process that gave all device memory to its own pool at start-up has
+ * none left to ask the driver for; a latency-bound loop cannot take the device-wide stall an allocation or free
+ * may cause.  Those callers already own their input and output arrays.  What they lack is a place for the round's
+ * split points, so this entry point keeps that scratch inside the library.
+ *
+ * The scratch and its limit.  The split points live in a fixed array of BCF_STATIC_MAX_SHARES uint32 (256 KiB)
+ * that is part of libbcf.so's device image: every GPU on which the library is used holds those 256 KiB from first
+ * use until the process exits, whether or not this function is ever called.  A round is accepted when
+ *      bcf_merge_round_static_shares(n, run_len) = ceil(n / (2 run_len)) * ceil(2 run_len / BCF_TILE)
+ * is at most BCF_STATIC_MAX_SHARES (n <= 2^26 elements when 2 run_len is a multiple of BCF_TILE); anything larger
+ * returns BCF_ERR_TOO_LARGE before any work is enqueued -- use bcf_merge_runs with a workspace for those.
+ *
+ * What it computes.  Runs are [i run_len, min(n, (i+1) run_len)), each already sorted (unchecked); runs 2p and 2p+1
+ * are merged into output positions [2p run_len, min(n, (2p+2) run_len)); an unpaired last run is copied.  The output
+ * therefore consists of sorted runs of 2 run_len: for n <= 2 run_len it is the result of bcf_merge_runs, and a
+ * caller with more runs repeats the call with run_len doubled, swapping its own two buffers (ceil(log2(#runs)) calls).
+ * Same kernels as bcf_merge_runs with BCF_MERGE_IMPL_GENERIC (exact co-rank partition, then one warp per page
+ * doing SHEARSORT-MERGE), same ordering contract, all four element types.
+ *   d_keys_in / d_vals_in   : n elements, not modified.      d_keys_out / d_vals_out : n elements, no overlap with the inputs.
+ *
+ * Things to know.
+ *  - No cudaMalloc, cudaFree or other allocating call is made, on the first call or later.  Two kernels are
+ *    enqueued on `stream`; the call does not synchronise.
+ *  - The FIRST call on each device does a one-off set-up with that device current: it checks the compute
+ *    capability, asks the runtime for the device address of the built-in array (cudaGetSymbolAddress) and opts the
+ *    merge kernels into their shared memory size.  Make that first call during start-up, before any stream capture
+ *    is begun; later calls only launch.  The set-up is thread-safe.
+ *  - All calls on a device share the one array, and it keeps whatever the previous call wrote.  Nothing in it has to
+ *    start at zero (every entry a round reads is written by that round's partition kernel first), so there is
+ *    nothing to clear.  But two calls whose kernels can run at the same time on one GPU -- different streams, or
+ *    different host threads on different streams -- overwrite each other's split points and produce garbage:
+ *    keep the calls of one device in one stream, or order them with events.
+ *  - The measurement hooks at the end of this file do not count or time these launches.
+ */
+#define BCF_STATIC_MAX_SHARES 65536
+size_t bcf_merge_round_static_max_shares(void);                 /* BCF_STATIC_MAX_SHARES, for callers that dlopen    */
+size_t bcf_merge_round_static_shares(size_t n, size_t run_len); /* split points one round needs; 0 for invalid sizes */
+bcf_status bcf_merge_round_static(const void *d_keys_in, const void *d_vals_in, void *d_keys_out, void *d_vals_out,
+                                  size_t n, size_t run_len, bcf_key_t kt, bcf_val_t vt, bcf_stream_t stream);
 
 /*
  * bcf_sort -- BCFMergesort (section 3, Appendix B): base case on

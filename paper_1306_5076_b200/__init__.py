@@ -43,6 +43,9 @@ from .binding import (  # noqa: F401
     LAUNCH_AUTO,
     LAUNCH_PLAIN,
     LAUNCH_PDL,
+    merge_round_static,
+    merge_round_static_max_shares,
+    merge_round_static_shares,
     merge_runs,
     merge_runs_pagewise,
     num_shares,

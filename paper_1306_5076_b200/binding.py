@@ -99,6 +99,11 @@ def lib():
     L.bcf_merge_runs.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_runs_pagewise.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp]
     L.bcf_merge_runs_ex.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp, sz, vp, vp]
+    L.bcf_merge_round_static_max_shares.restype = sz
+    L.bcf_merge_round_static_max_shares.argtypes = []
+    L.bcf_merge_round_static_shares.restype = sz
+    L.bcf_merge_round_static_shares.argtypes = [sz, sz]
+    L.bcf_merge_round_static.argtypes = [vp, vp, vp, vp, sz, sz, ci, ci, vp]
     L.bcf_sort.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
     L.bcf_sort_ex.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp, vp]
     L.bcf_sort_host.argtypes = [vp, vp, sz, ci, ci, vp, sz, vp]
@@ -324,6 +329,30 @@ def merge_runs_pagewise(keys, run_len, vals=None, out_keys=None, out_vals=None, 
     """bcf_merge_runs_pagewise: the paper's streaming Alg. 6, one warp per pair of runs."""
     return _merge(lib().bcf_merge_runs_pagewise, "bcf_merge_runs_pagewise", OP_MERGE_PAGEWISE, keys, run_len, vals,
                   out_keys, out_vals, workspace, stream)
+
+
+def merge_round_static_max_shares():
+    """bcf_merge_round_static_max_shares: size of the library's built-in split-point array (entries)."""
+    return int(lib().bcf_merge_round_static_max_shares())
+
+
+def merge_round_static_shares(n, run_len):
+    """bcf_merge_round_static_shares: split points one round of (n, run_len) needs; 0 for invalid sizes."""
+    return int(lib().bcf_merge_round_static_shares(int(n), int(run_len)))
+
+
+def merge_round_static(keys, run_len, out_keys, vals=None, out_vals=None, stream=None):
+    """bcf_merge_round_static: one merge round (runs 2p, 2p+1 -> a run of 2 run_len) for callers that cannot
+    allocate device memory where they merge.  The library brings its own split-point scratch (a fixed 256 KiB
+    array per GPU), so this wrapper allocates nothing either: the caller passes every tensor, outputs included.
+    Rounds needing more than merge_round_static_max_shares() split points raise BcfError(BCF_ERR_TOO_LARGE).
+    Calls on one GPU share that scratch: keep them on one stream.  The first call per device does a one-off
+    set-up; make it before any stream capture."""
+    kt, vt = _types(keys, vals)
+    _check(lib().bcf_merge_round_static(_dev(keys, "keys"), _dev(vals, "vals"), _dev(out_keys, "out_keys"),
+                                        _dev(out_vals, "out_vals"), keys.numel(), int(run_len), kt, vt, _stream(stream)),
+           "bcf_merge_round_static")
+    return out_keys if vals is None else (out_keys, out_vals)
 
 
 def sort(keys, vals=None, workspace=None, stream=None, opts=None):

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libbcf.so")
 SOURCES = ["bcf_api.cu", "bcf_tu_tile.cu", "bcf_tu_long.cu", "bcf_tu_merge.cu", "bcf_tu_pipe.cu", "bcf_tu_merge4.cu",
-           "bcf_tu_buckets.cu", "bcf_tu_isolate.cu"]
+           "bcf_tu_buckets.cu", "bcf_tu_isolate.cu", "bcf_tu_static.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",

@@ -530,6 +530,7 @@ const char *bcf_status_string(bcf_status s)
     case BCF_ERR_WORKSPACE_TOO_SMALL: return "BCF_ERR_WORKSPACE_TOO_SMALL";
     case BCF_ERR_UNSUPPORTED_DEVICE: return "BCF_ERR_UNSUPPORTED_DEVICE";
     case BCF_ERR_CUDA: return "BCF_ERR_CUDA";
+    case BCF_ERR_TOO_LARGE: return "BCF_ERR_TOO_LARGE";
     }
     return "BCF_ERR_UNKNOWN";
 }
