@@ -29,8 +29,9 @@
  *    and is not left pending.  After a failure the contents of the output and workspace are unspecified.
  *  - STATE: the library keeps no settings.  Everything that selects an algorithm is passed per call in a
  *    bcf_options (below); two threads, or two calls, with different options do not interact.  The only
- *    process-wide state is the measurement hooks at the end of this file (not thread-safe, off by
- *    default) and per-device caches of kernel attributes (thread-safe, keyed by device id).
+ *    process-wide state is the measurement hooks at the end of this file (timing: not thread-safe, off by
+ *    default, and untouched by calls made while it is off; launch counts: atomic counters, safe from any
+ *    number of threads) and per-device caches of kernel attributes (thread-safe, keyed by device id).
  *  - DEVICE: compute capability 10.x (B200, sm_100a) is required; anything else returns
  *    BCF_ERR_UNSUPPORTED_DEVICE.  There is no fallback path of any kind.
  *  - LIMIT: n < 2^32 elements.
@@ -364,6 +365,8 @@ bcf_status bcf_sort_ex(void *d_keys, void *d_vals, size_t n, bcf_key_t kt, bcf_v
  * If one run remains after phase 2 the result is complete and phases 3-4 are skipped.
  *   d_keys      : n keys, sorted in place.
  *   P, t        : buckets and samples per run; 2 <= P <= 65536, 1 <= t <= 65536 (the paper: t = P = 128).
+ *                 Where the s runs left by phase 2 give fewer than P samples (s t < P), t is raised to
+ *                 ceil(P / s) for this call; the workspace size below already accounts for that.
  *   d_workspace : >= bcf_sort_buckets_workspace_bytes(n, t, P, pivot_buckets, kt) bytes.
  *   d_bucket_starts : NULL, or nb + 1 uint32 (device): start of every bucket in the sorted output, last = n
  *                 (nb = P or 2P-1); written only when phases 3-4 ran (n > P runs of one tile, more than one run).

@@ -120,7 +120,9 @@ struct Profile {
     int created = 0;
     int open_since = -1;               // first entry of the API call in progress
     unsigned long long dropped = 0;    // launches not timed because the pool was full
-    unsigned long long launches[BCF_KERNEL_CLASSES] = {0, 0, 0, 0};
+    // launch counts are kept whether or not timing is on, by every thread that launches: relaxed atomics.
+    // Everything else in this struct is touched only while timing is on (one thread, include/bcf.h).
+    std::atomic<unsigned long long> launches[BCF_KERNEL_CLASSES];
 } g_prof;
 
 inline int profile_mark(int cls, cudaStream_t s)
@@ -141,7 +143,7 @@ inline int profile_mark(int cls, cudaStream_t s)
 
 void bcf::profile_launch(int cls, cudaStream_t stream)
 {
-    g_prof.launches[cls]++;
+    g_prof.launches[cls].fetch_add(1, std::memory_order_relaxed);
     profile_mark(cls, stream);
 }
 
@@ -151,13 +153,13 @@ namespace {
 struct ProfileGroup {
     cudaStream_t s;
     bool outer;
-    explicit ProfileGroup(cudaStream_t stream) : s(stream), outer(g_prof.open_since < 0)
+    explicit ProfileGroup(cudaStream_t stream) : s(stream), outer(g_prof.on && g_prof.open_since < 0)
     {
         if (outer) g_prof.open_since = g_prof.used;
     }
     ~ProfileGroup()
     {
-        if (!outer) return;
+        if (!outer) return;              // timing off: concurrent callers share no state here
         if (g_prof.used > g_prof.open_since && g_prof.cls[g_prof.used - 1] >= 0) profile_mark(-1, s);
         g_prof.open_since = -1;
     }
@@ -752,6 +754,15 @@ static size_t buckets_stop_len(size_t n, size_t base_run, int P)
     return l;
 }
 
+// Samples per run the distribution really takes on runs of stop_len: the caller's t, raised to ceil(P / s) where
+// s t < P (Alg. 7 needs at least P samples to choose P - 1 pivots from).  The workspace is sized with the same value.
+static int buckets_samples_per_run(size_t n, size_t stop_len, int t, int P)
+{
+    const size_t s = (n + stop_len - 1) / stop_len;
+    if (s * static_cast<size_t>(t) >= static_cast<size_t>(P)) return t;
+    return static_cast<int>((static_cast<size_t>(P) + s - 1) / s);
+}
+
 // [keys copy W1][piece offsets][pivots][max(sort workspace, FIND-BUCKETS workspace, final-phase workspace)]
 struct BucketsWs {
     size_t w1, offsets, pivots, rest, total;
@@ -770,7 +781,7 @@ static BucketsWs buckets_ws(size_t n, int t, int P, int pb, bcf_key_t kt)
     size_t fb = 0;
     for (size_t base : {size_t(TILE), size_t(BCF_LONG_TILE_H) * TILE}) {
         const size_t l = buckets_stop_len(n, base, P);
-        const size_t v = bcf_find_buckets_workspace_bytes(n, l, t, P, pb, kt);
+        const size_t v = bcf_find_buckets_workspace_bytes(n, l, buckets_samples_per_run(n, l, t, P), P, pb, kt);
         if (v > fb) fb = v;
     }
     if (fb > rest) rest = fb;
@@ -826,9 +837,10 @@ bcf_status bcf_sort_buckets(void *d_keys, size_t n, bcf_key_t kt, int t, int P, 
 
     // phase 3: FIND-BUCKETS  d_keys -> W1
     BucketsGeom g;
-    int tt = t;
-    if (s * static_cast<size_t>(tt) < static_cast<size_t>(P)) tt = static_cast<int>((P + s - 1) / s);   // s t >= P
+    const int tt = buckets_samples_per_run(n, stop_len, t, P);                                           // s t >= P
     if (!buckets_geom(n, stop_len, tt, P, pivot_buckets, &g)) return BCF_ERR_INVALID_ARG;
+    if (bcf_find_buckets_workspace_bytes(n, stop_len, tt, P, pivot_buckets, kt) > w.total - w.rest)
+        return BCF_ERR_WORKSPACE_TOO_SMALL;      // cannot happen while buckets_ws sizes `rest` with the same tt
     st = find_buckets_impl(c, d_keys, g, kt, w1, pivots, offsets, rest);
     if (st != BCF_OK) return st;
     if (d_bucket_starts)
@@ -1063,8 +1075,8 @@ unsigned long long bcf_profile_dropped(void) { return g_prof.dropped; }
 void bcf_launch_counts(unsigned long long *launches)
 {
     for (int c = 0; c < BCF_KERNEL_CLASSES; ++c) {
-        if (launches) launches[c] = g_prof.launches[c];
-        g_prof.launches[c] = 0;
+        const unsigned long long v = g_prof.launches[c].exchange(0, std::memory_order_relaxed);
+        if (launches) launches[c] = v;
     }
 }
 

@@ -262,3 +262,28 @@ def test_argument_errors_are_reported_before_any_device_work():
     assert L.bcf_sort_buckets(p, 0, 0, 4, 4, 0, None, None, 0, None, None) == 0
     assert L.bcf_merge_pieces_workspace_bytes(1 << 14, 4, 1, 0) > 0 and L.bcf_merge_pieces_workspace_bytes(0, 4, 4, 0) == 0
     assert L.bcf_merge_pieces(p, p, 100, p, 4, 4, 0, 0, p, 1 << 14, None) == INVALID            # in/out aliasing
+
+
+@pytest.mark.parametrize("kt,P,t,pb,n", [(1, 4096, 1, 1, 4095 * 1024 - 5), (0, 2048, 1, 0, 2047 * 1024 - 5),
+                                         (0, 2048, 1, 1, 2048 * 1024 - 3), (1, 128, 128, 1, 1 << 22), (0, 4096, 3, 1, 3000 * 1024)])
+def test_sort_buckets_workspace_covers_the_distribution_when_t_is_raised(kt, P, t, pb, n):
+    """bcf_sort_buckets raises t to ceil(P / s) where the s runs of phase 2 give fewer than P samples; its
+    workspace must be sized with that same t (r2 advisor: with t = 1 and a large P the FIND-BUCKETS region was
+    sized as 0 bytes and the call wrote ~34 MB past the caller's workspace).  Host arithmetic only: the region
+    after [keys copy][piece offsets][pivots] must hold bcf_find_buckets_workspace_bytes for both base run lengths."""
+    L = binding.lib()
+    total = L.bcf_sort_buckets_workspace_bytes(n, t, P, pb, kt)
+    assert total > 0
+    up = lambda x: (x + 255) // 256 * 256      # noqa: E731
+    kb = 8 if kt else 4
+    nb = 2 * P - 1 if pb else P
+    rest_off = up(n * kb) + up((nb * P + 1) * 4) + up(P * kb)
+    for base in (1024, 8192):
+        run = base
+        while -(-n // run) > P:
+            run *= 2
+        s = -(-n // run)
+        tt = t if s * t >= P else -(-P // s)
+        need = L.bcf_find_buckets_workspace_bytes(n, run, tt, P, pb, kt)
+        assert need > 0
+        assert total - rest_off >= need, (base, s, tt, total - rest_off, need)

@@ -540,6 +540,26 @@ def test_sort_buckets_matches_oracle(bcf, kind, pb, n, P, t, data, base):
     assert np.array_equal(host(d, keys), want)
 
 
+@pytest.mark.parametrize("kind,P,n", [("u32", 2048, 2047 * 1024 - 5), ("u64", 2048, 2047 * 1024 - 5), ("u32", 1024, 1023 * 1024 + 1)])
+@pytest.mark.parametrize("pb", [False, True], ids=["plain", "pivot_buckets"])
+def test_sort_buckets_few_samples_stays_inside_its_workspace(bcf, kind, P, n, pb, base):
+    """t = 1 with a large P: the s <= P runs left by the first merge phase give fewer than P samples, so the call
+    raises t to ceil(P / s).  The workspace is exactly bcf_sort_buckets_workspace_bytes(n, t = 1, ...) followed by a
+    guard region; the output is the unique sorted sequence (vs numpy's sort) and the guard is untouched."""
+    dt = np.uint32 if kind == "u32" else np.uint64
+    rng = np.random.default_rng(n + P)
+    keys = rng.integers(0, 1 << 32, size=n, dtype=np.uint64).astype(dt)
+    if kind == "u64":
+        keys = (keys << np.uint64(32)) | rng.integers(0, 1 << 32, size=n, dtype=np.uint64)
+    need = int(bcf.lib().bcf_sort_buckets_workspace_bytes(n, 1, P, int(pb), 0 if kind == "u32" else 1))
+    guard = 64 << 20
+    buf = torch.full((need + guard,), 0xA5, dtype=torch.uint8, device="cuda")
+    d = dev(keys)
+    bcf.sort_buckets(d, P, t=1, pivot_buckets=pb, workspace=buf[:need], opts={"base_case": base})
+    assert np.array_equal(host(d, keys), np.sort(keys))
+    assert bool((buf[need:] == 0xA5).all())
+
+
 def test_sort_buckets_bucket_starts_match_oracle_and_lemma_1(bcf):
     """The distribution inside bcf_sort_buckets is the oracle's (same runs, same pivots): bucket starts equal,
     and with all keys distinct no bucket exceeds Lemma 1's bound s ceil(N/(s t)) + ceil(s t/P) ceil(N/(s t))."""
