@@ -39,12 +39,30 @@ def _compile(nvcc, src, obj, verbose, extra):
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), log=None) -> str:
-    """Compile what is out of date and link.  `extra_flags` (e.g. -D...) are for A/B experiments only; they force
-    a full rebuild.  `log`: file that receives the compiler output (ptxas -v lines with verbose)."""
+    """Compile what is out of date and link.  `extra_flags` (e.g. -D...) are for A/B experiments only.  The flag set
+    of the objects under build/ is recorded in build/flags.stamp; whenever it differs from this call's flags (in
+    either direction) every unit is recompiled.  `log`: file that receives the compiler output (ptxas -v lines with
+    verbose)."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ, exist_ok=True)
     hdr = _headers_mtime()
-    force = force or bool(extra_flags)
+    # The objects in build/ belong to ONE flag set.  Its record sits beside them; a build with other flags (an A/B
+    # experiment with -D..., or the plain build that follows one) recompiles every unit instead of linking stale
+    # objects of the other kernel shape into libbcf.so.
+    flags_now = " ".join(NVCC_FLAGS + list(extra_flags))
+    stamp = os.path.join(OBJ, "flags.stamp")
+    try:
+        with open(stamp) as f:
+            flags_then = f.read()
+    except OSError:
+        flags_then = None
+    if flags_then != flags_now:
+        force = True
+        for stale in [OUT] + [os.path.join(OBJ, f) for f in os.listdir(OBJ) if f.endswith(".o")]:
+            if os.path.exists(stale):   # nothing of the other flag set survives, even if this build fails half-way
+                os.remove(stale)
+        with open(stamp, "w") as f:
+            f.write(flags_now)
     todo = []
     for s in SOURCES:
         src = os.path.join(CSRC, s)
