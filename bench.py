@@ -145,6 +145,31 @@ class Job:
             ok = bool(np.all(out[:-1] <= out[1:]))
         if not ok:
             raise SystemExit(f"bench: output of {self.name} not sorted")
+        # the same multiset as the input, by two order-independent checksums (a lost or duplicated key changes them)
+        if _multiset_checksum(out) != _multiset_checksum(self.host_keys):
+            raise SystemExit(f"bench: output keys of {self.name} are not a permutation of the input")
+        if self.host_vals is not None and self.v is not None:
+            if _multiset_checksum(self.v.cpu().numpy().view(np.uint32)) != _multiset_checksum(self.host_vals):
+                raise SystemExit(f"bench: output values of {self.name} are not a permutation of the input")
+
+
+def _multiset_checksum(a):
+    """(sum mod 2^64, xor) of an unsigned integer array: equal for equal multisets, whatever the order."""
+    a = np.ascontiguousarray(a)
+    return int(a.sum(dtype=np.uint64)), int(np.bitwise_xor.reduce(a))
+
+
+def _device_sorted_unsigned(torch, d):
+    """d (an int32 / int64 tensor holding unsigned bit patterns) is ascending as UNSIGNED integers: flipping the
+    sign bit maps unsigned order onto signed order."""
+    flip = d ^ torch.iinfo(d.dtype).min
+    return bool((flip[1:] >= flip[:-1]).all().item())
+
+
+def _device_checksum(torch, d):
+    """Order-independent checksums of a device tensor (wrapping 64-bit sums of x and of x * x)."""
+    x = d.to(torch.int64)
+    return int(x.sum().item()), int((x * x).sum().item())
 
 
 def measured_peak():
@@ -357,8 +382,11 @@ def sort_buckets_lines(bcf, torch, dev, stream):
                 d.copy_(src)
                 fn()
             torch.cuda.synchronize()
-            if not bool((d[1:] >= d[:-1]).all().item()) and dname != "uniform keys":
-                raise SystemExit("bench: sort_buckets output not sorted")
+            # once per variant, after warm-up, for both inputs: sorted as unsigned keys, same multiset as the input
+            if not _device_sorted_unsigned(torch, d):
+                raise SystemExit("bench: sort_buckets output not sorted (%s, %s)" % (dname, label))
+            if _device_checksum(torch, d) != _device_checksum(torch, src):
+                raise SystemExit("bench: sort_buckets output is not a permutation of the input (%s, %s)" % (dname, label))
             bcf.launch_counts()
             ms = []
             for _ in range(5):
@@ -454,6 +482,30 @@ def colored_scan_lines(bcf, torch, dev, stream):
     return lines
 
 
+# comparators per element of the two tile networks (include/bcf.h): ShearSort = 11 line sorts x 191 comparators per
+# 32-element line; tile mergesort = 831 comparators per thread per tile of 32 x 32
+TILE_COMPARATORS_PER_ELEMENT = {"shearsort": 11 * 191 / 32, "mergesort": 831 / 32}
+# ALU-pipe instructions per comparator, from the SASS: u32 = VIMNMX min + max = 2; two planes = 2 subtract-with-
+# borrow (IADD3 / IADD3.X into a predicate) + 3 SEL = 5 (the fourth output is formed with 2 IMADs on the FMA
+# pipe, BCF_CE2_FMA_PLANES = 1); three planes = 3 + 6 SEL = 9
+ALU_OPS_PER_COMPARATOR = {"u32": 2, "u32+u32": 5, "u64": 5, "u64+u32": 9}
+
+
+def alu_roofline(dtype, n, tile_algo, launch_ms, sm_max_mhz=None):
+    """SURVEY.md 8(d)'s second ceiling for the batch tile sorts (configs 1-2): ALU-pipe instructions the network
+    issues (comparators x instructions per comparator, as built) over the launch's event time, against
+    148 SMs x 64 integer lanes per clock x the SM's maximum clock."""
+    sm_mhz = sm_max_mhz or 1965.0
+    ops = n * TILE_COMPARATORS_PER_ELEMENT[tile_algo] * ALU_OPS_PER_COMPARATOR[dtype]
+    peak_ops = 148 * 64 * sm_mhz * 1e6
+    ach = ops / (launch_ms * 1e-3)
+    kernel = "tile_sort_kernel (ShearSort)" if tile_algo == "shearsort" else "tile_mergesort_kernel"
+    return {"kernel": kernel + ", one launch = all tiles", "bound": "alu", "achieved": ach / 1e12, "peak": peak_ops / 1e12,
+            "unit": "T int-op/s", "frac": ach / peak_ops,
+            "alu_ops_per_element": TILE_COMPARATORS_PER_ELEMENT[tile_algo] * ALU_OPS_PER_COMPARATOR[dtype],
+            "peak_source": "148 SMs x 64 integer min/max lanes per clk x SM max clock %.0f MHz (DESIGN.md 5.1)" % sm_mhz}
+
+
 def _side_line(bcf, torch, dev, name, stream, barrier, variant):
     desc, logn, gen, op, dtype = WORKLOADS[name]
     n = 1 << logn
@@ -478,6 +530,8 @@ def _side_line(bcf, torch, dev, name, stream, barrier, variant):
             "ms_per_step": t, "best_ms": min(ms), "passes": passes,
             "frac_of_measured_hbm_peak_for_pass_count": bytes_moved / (t * 1e-3) / 1e9 / peak,
             "gpu_launches_per_step": int(sum(launches.values())) // 5}
+    if op == "tiles":      # one launch per step: the step's event time is the launch's
+        line["alu_roofline"] = alu_roofline(dtype, n, TILE_ALGO, t)
     if variant:
         line["variant"] = variant.get("label", "")
     del job
@@ -585,18 +639,9 @@ def main():
     if dom == "tile_sort" and op == "tiles":
         # ALU-bound: 11 line sorts x 191 comparators x 2 min/max per 32 u32 keys,
         # integer min/max issue at 64 lanes / clk / SM.
-        sm_mhz = clocks.get("sm_max_mhz") or 1965.0
-        # ALU-pipe instructions per comparator, from the SASS: u32 = VIMNMX min + max = 2; two planes = 2 subtract-with-
-        # borrow (IADD3 / IADD3.X into a predicate) + 3 SEL = 5 (the fourth output is formed with 2 IMADs on the FMA
-        # pipe, BCF_CE2_FMA_PLANES = 1); three planes = 3 + 6 SEL = 9
-        ops = n * 11 * 191 / 32 * {"u32": 2, "u32+u32": 5, "u64": 5, "u64+u32": 9}[dtype]
-        peak_ops = 148 * 64 * sm_mhz * 1e6
-        ach = ops / (d_ms / d_cnt * 1e-3)
-        roofline = {"kernel": "tile_sort_kernel (one launch = ShearSort of all tiles)", "bound": "alu",
-                    "achieved": ach / 1e12, "peak": peak_ops / 1e12, "unit": "T int-op/s", "frac": ach / peak_ops,
-                    "traffic": recorded_traffic("tile_sort"),
-                    "peak_source": "148 SMs x 64 integer min/max lanes per clk x SM max clock (DESIGN.md 5.1)",
-                    "launches_timed": d_cnt, "mean_launch_ms": d_ms / d_cnt, "share_of_step": share}
+        roofline = alu_roofline(dtype, n, TILE_ALGO, d_ms / d_cnt, clocks.get("sm_max_mhz"))
+        roofline.update({"traffic": recorded_traffic("tile_sort"), "launches_timed": d_cnt, "mean_launch_ms": d_ms / d_cnt,
+                         "share_of_step": share})
     else:
         m_ms, m_cnt = prof["merge"]
         achieved = alg_bytes / (m_ms / m_cnt * 1e-3) / 1e9 if m_cnt else None
@@ -686,6 +731,8 @@ def main():
         for ln in side:
             if ln["workload"] in SIDE_WORKLOADS and "variant" not in ln:
                 summary[ln["workload"]] = [round(ln["value"] / 1e9, 2), round(ln["frac_of_measured_hbm_peak_for_pass_count"], 3)]
+                if "alu_roofline" in ln:    # configs 1-2: also the fraction of the ALU ceiling (third entry)
+                    summary[ln["workload"]].append(round(ln["alu_roofline"]["frac"], 3))
         kv5a = next(ln for ln in side if ln["workload"] == "cfg5a" and "variant" not in ln)
         kv = {"workload": "cfg5a", "dtype": kv5a["dtype"], "n": kv5a["n"], "value": kv5a["value"], "unit": UNIT,
               "ms_per_step": kv5a["ms_per_step"], "passes": kv5a["passes"],
