@@ -193,7 +193,7 @@ def recorded_traffic(kernel):
 
 def recorded_bank_conflicts():
     """Shared-memory bank-conflict counters per kernel of the committed ncu capture of THIS build
-    (profiles/bank_conflicts.json, written from the ncu CSV by the command named in profiles/r2_conflicts.md):
+    (profiles/bank_conflicts.json, written from the ncu CSV by the command named in profiles/r3_launches.md; its `build` entry says which build):
     {kernel: {ld, st, wavefronts_ld, wavefronts_st, excess_per_instruction}}; None when no capture is committed."""
     path = os.path.join(ROOT, "profiles", "bank_conflicts.json")
     try:
@@ -640,7 +640,7 @@ def main():
         # ALU-bound: 11 line sorts x 191 comparators x 2 min/max per 32 u32 keys,
         # integer min/max issue at 64 lanes / clk / SM.
         roofline = alu_roofline(dtype, n, TILE_ALGO, d_ms / d_cnt, clocks.get("sm_max_mhz"))
-        roofline.update({"traffic": recorded_traffic("tile_sort"), "launches_timed": d_cnt, "mean_launch_ms": d_ms / d_cnt,
+        roofline.update({"traffic": recorded_traffic("tile_sort_shearsort_cfg2") if args.workload == "cfg2" and TILE_ALGO == "shearsort" else None, "launches_timed": d_cnt, "mean_launch_ms": d_ms / d_cnt,
                          "share_of_step": share})
     else:
         m_ms, m_cnt = prof["merge"]
