@@ -48,8 +48,8 @@ extern "C" {
 
 #define BCF_W 32            /* warp size = number of 4-byte shared memory banks */
 #define BCF_TILE 1024       /* M = w*w elements per tile / page           */
-#define BCF_SHARE 8192      /* outputs per share of the four-run pass (bcf_merge_partition4) and of the
-                               isolation experiment: 8 pages.  The two-run merge kernel picks its own share
+#define BCF_SHARE 8192      /* outputs per share of the four-run pass (bcf_merge_partition4): 8 pages.
+                               The two-run merge kernel picks its own share
                                size per element type (16 / 4 / 8 pages for 4- / 8- / 12-byte elements).       */
 
 /* A CUDA stream handle; identical to cudaStream_t / CUstream. */
@@ -416,14 +416,15 @@ bcf_status bcf_merge_runs_pagewise(const void *d_keys_in, const void *d_vals_in,
 /* ------------------------------------------------------------------ debug: conflict isolation --- */
 
 /*
- * The bank-conflict isolation experiment (csrc/bcf_tu_isolate.cu; profiles/r2_conflict_isolation.md).  DEBUG entry
+ * The bank-conflict isolation experiment (csrc/bcf_tu_isolate.cu; profiles/r3_conflict_isolation.md).  DEBUG entry
  * points: nothing in the library calls them.  They run the same shared-memory instruction streams as
  * merge_pipe_kernel and tile_mergesort_kernel (uint32 keys) in three phases separated by CTA barriers --
  * global -> chip, every LDS / STS of the work item, registers -> global -- so that ncu's
  * l1tex__data_bank_conflicts_pipe_lsu_mem_shared_op_{ld,st} can be read with (exclusive = 0, several CTAs per SM)
  * and without (exclusive = 1, one CTA per SM) other global-memory traffic on the SM during the LDS / STS phase.
- *   bcf_debug_merge_round_isolated : ONE merge round of runs of run_len = 8192 * 2^k; n a multiple of
- *       2 run_len; out of place; d_workspace >= (n / BCF_SHARE + 1) * 4 bytes (split points, production kernel).
+ *   bcf_debug_merge_round_isolated : ONE merge round of runs of run_len = 16384 * 2^k (at least one share
+ *       of the production uint32 merge kernel, whose shape -- 16-page shares, 16 warps, one CTA per SM -- it copies); n a
+ *       multiple of 2 run_len; out of place; d_workspace >= (n / BCF_SHARE + 1) * 4 bytes (split points, production kernel).
  *   bcf_debug_sort_tiles_isolated  : bcf_sort_tiles_mergesort of whole tiles, in place.
  * Results are those of bcf_merge_runs / bcf_sort_tiles (parity-tested).
  */

@@ -1,4 +1,4 @@
-"""The bank-conflict isolation experiment (profiles/r2_conflict_isolation.md).
+"""The bank-conflict isolation experiment (profiles/r3_conflict_isolation.md).
 
     python -m paper_1306_5076_b200.conflict_isolation [--log2n 24]
 
@@ -10,7 +10,8 @@ l1tex__data_bank_conflicts_pipe_lsu_mem_shared_op_st.sum,...` pass over this scr
   tile_mergesort_isolated_kernel  (grid B)   same code, several CTAs per SM (phases of different CTAs overlap)
   merge_pipe_kernel                          production, TMA producer + consumers + stores overlap
   merge_round_isolated_kernel     (grid A)   phases separated, ONE CTA per SM                    -> expected 0
-  merge_round_isolated_kernel     (grid B)   same code, two CTAs per SM
+  merge_round_isolated_kernel     (grid B)   the same launch again: the experiment has the production shape (16-page
+                                             shares, 16 warps, one CTA per SM is all that fits), `exclusive` changes nothing
 Every output is checked against the production result before the script exits (exit code 1 on a mismatch).
 Launch order = the order above; the isolated kernels appear twice in ncu's list, exclusive (A) first.
 """

@@ -1011,7 +1011,7 @@ bcf_status bcf_debug_merge_round_isolated(const void *d_keys_in, void *d_keys_ou
                                           void *d_workspace, size_t workspace_bytes, bcf_stream_t stream)
 {
     if (n == 0) return BCF_OK;
-    if (n >= (size_t(1) << 32) || run_len < BCF_SHARE || (run_len & (run_len - 1)) || n % (2 * run_len)) return BCF_ERR_INVALID_ARG;
+    if (n >= (size_t(1) << 32) || run_len < isolated_share() || (run_len & (run_len - 1)) || n % (2 * run_len)) return BCF_ERR_INVALID_ARG;
     if (!d_keys_in || !d_keys_out || !d_workspace) return BCF_ERR_INVALID_ARG;
     if (!aligned16(d_keys_in) || !aligned16(d_keys_out) || !aligned16(d_workspace)) return BCF_ERR_MISALIGNED;
     if (overlap(d_keys_in, n * 4, d_keys_out, n * 4)) return BCF_ERR_INVALID_ARG;

@@ -14,7 +14,10 @@
 // With `exclusive` = 1 the launch asks for enough dynamic shared memory that ONE CTA is resident per SM, so no other
 // CTA's phase 1 / 3 can overlap this CTA's phase 2: if the counter is caused by arbitration it must read 0.  With
 // `exclusive` = 0 the same code runs with several CTAs per SM (their phases interleave): the counter must come back.
-// profiles/r2_conflict_isolation.md holds the measured table.
+// (The merge round has the production shape since r3 -- 16-page shares, 16 warps, ~196 KB of shared memory -- so one
+// CTA per SM is all that fits and `exclusive` makes no difference for it; the production kernel it is compared with
+// is also one CTA per SM, whose TMA writes and global stores overlap its own LDS / STS.)
+// profiles/r3_conflict_isolation.md holds the measured table (r2_conflict_isolation.md: the older 8-page shape).
 #include "bcf_internal.cuh"
 #include "bcf_merge_pipe.cuh"
 
@@ -22,12 +25,15 @@ namespace bcf {
 namespace isolate {
 
 using E = Elem<1, false>;
-// the shape of the experiment is fixed here, whatever the production kernel uses: shares of 8 pages, one page per warp,
-// two stage buffers (profiles/r2_conflict_isolation.md was measured with exactly this)
-constexpr int NW = 8;
-constexpr int SH = NW * TILE;
-constexpr int NSTAGE = 2;
+// the shape of the experiment follows the production merge kernel for uint32 keys (pipe::Cfg<E>): the same share size
+// (16 pages), one page per consumer warp (16 warps), two stage buffers -- so ONE CTA fills an SM here exactly as in
+// merge_pipe_kernel<u32>, and whatever the production counter shows comes from that CTA's own concurrent traffic
+// (TMA writes into the stage buffers, STG data), not from a neighbour CTA.
+constexpr int NW = pipe::Cfg<E>::PAGES;
+constexpr int SH = pipe::Cfg<E>::SH;
+constexpr int NSTAGE = pipe::Cfg<E>::STAGES;
 constexpr int THREADS = NW * 32;
+static_assert(NW == pipe::Cfg<E>::NWC, "one consumer warp per page, as in the production kernel");
 struct C {
     static constexpr size_t stage_bytes = size_t(SH) * 4 + pipe::REGION_SLACK;
     static constexpr size_t scratch_off = NSTAGE * stage_bytes;
@@ -35,9 +41,10 @@ struct C {
     static constexpr size_t bar_off = meta_off + NSTAGE * sizeof(pipe::ShareMeta);
     static constexpr size_t total = bar_off + NSTAGE * 8;
 };
+static_assert(C::total + 1024 <= 227 * 1024, "the experiment's CTA must fit one SM");
 constexpr size_t EXCLUSIVE_SMEM = 120 * 1024;      // more than half of the 227 KB an SM offers: one CTA per SM
 
-// One merge round on u32 keys, runs of L = 1024 * 2^k >= 8192, n a multiple of 8192: each CTA merges NSTAGE shares.
+// One merge round on u32 keys, runs of L = 1024 * 2^k >= SH, n a multiple of 2 L: each CTA merges NSTAGE shares.
 __global__ void __launch_bounds__(THREADS, 1)
 merge_round_isolated_kernel(const uint32_t *__restrict__ kin, uint32_t *__restrict__ kout, const uint32_t *__restrict__ splits,
                             const unsigned long long n, const unsigned long long L, const unsigned long long num_shares)

@@ -135,7 +135,7 @@ def main():
                        "excess_per_instruction = sum over the kernel's LDS/STS of (L1 wavefronts shared - ideal) on the source "
                        "page of that kernel's --set full capture (excess_from), null for a kernel with no such capture; "
                        "the kernel-level counters are not per-instruction conflicts but arbitration with the SM's other "
-                       "shared-memory and global traffic (profiles/r2_conflict_isolation.md)",
+                       "shared-memory and global traffic (profiles/r3_conflict_isolation.md)",
                "kernels": out}
         with open(args.json, "w") as f:
             json.dump(doc, f, indent=1)
