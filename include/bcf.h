@@ -34,7 +34,8 @@
  *    number of threads) and per-device caches of kernel attributes (thread-safe, keyed by device id).
  *  - DEVICE: compute capability 10.x (B200, sm_100a) is required; anything else returns
  *    BCF_ERR_UNSUPPORTED_DEVICE.  There is no fallback path of any kind.
- *  - LIMIT: n < 2^32 elements.
+ *  - LIMIT: n < 2^32 elements.  Largest inputs tested on a B200 (tests/test_gpu_fullsize.py): 2^31 + 4099 uint32
+ *    keys and 2^30 + 77 (uint64, uint32) pairs through bcf_sort.
  */
 #ifndef BCF_H_
 #define BCF_H_

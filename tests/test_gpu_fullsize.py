@@ -68,7 +68,7 @@ def test_config3_full_size_exact(bcf):
 
 
 @pytest.mark.parametrize("dist", workloads.CFG4_VARIANTS)
-def test_config4_full_size(bcf, dist):
+def test_config4_full_size_vs_numpy_sort_unique_result(bcf, dist):
     """2^28 uint32 keys, each of the five distributions."""
     keys = workloads.cfg4_sort_u32(dist)
     d = dev(keys)
@@ -95,7 +95,7 @@ def test_config4_full_size_paper_base_case_and_two_rounds_per_pass(bcf):
 
 
 @pytest.mark.parametrize("data", ["zero_one", "dup256", "uniform"])
-def test_sort_buckets_full_size(bcf, data):
+def test_sort_buckets_full_size_vs_numpy_sort_unique_result(bcf, data):
     """BCFMergesort with the paper's distribution (t = P = 128, the paper's p) and BCFMergesortPB at 2^27 keys
     (the size of bench.py's side line): every element against numpy's sort; 0-1 data is the paper's 15.5x case."""
     n = 1 << 27
@@ -115,7 +115,7 @@ def test_sort_buckets_full_size(bcf, data):
         torch.cuda.empty_cache()
 
 
-def test_config5a_full_size(bcf):
+def test_config5a_full_size_by_the_properties_that_fix_the_unique_result(bcf):
     """2^26 (u64 key, u32 value = index) pairs: the properties determine the output uniquely."""
     keys, vals = workloads.cfg5a_sort_u64_u32()
     dk, dv = dev(keys), dev(vals)
@@ -124,7 +124,7 @@ def test_config5a_full_size(bcf):
 
 
 @pytest.mark.parametrize("k", [2, 64, 1024])
-def test_config5b_full_size(bcf, k):
+def test_config5b_full_size_vs_numpy_sort_unique_result(bcf, k):
     """merge-only: k sorted runs totalling 2^27 uint32 keys."""
     keys, run_len = workloads.cfg5b_merge_runs_u32(k)
     out = host(bcf.merge_runs(dev(keys), run_len), keys)
@@ -149,3 +149,64 @@ def test_config2_full_size_sampled_tiles(bcf):
             sl = slice(1024 * t, 1024 * (t + 1))
             wk, wv = oracle.shearsort_tiles(keys[sl], vals[sl])
             assert np.array_equal(ok[sl], wk) and np.array_equal(ov[sl], wv)
+
+
+# ---------------------------------------------------------------- the size range include/bcf.h promises (n < 2^32)
+
+
+def _flip(t):
+    """int tensor holding unsigned bit patterns -> same tensor with unsigned order mapped onto signed order."""
+    return t ^ torch.iinfo(t.dtype).min
+
+
+def test_sort_more_than_2_pow_31_uint32_keys_by_rank_counting(bcf):
+    """n = 2^31 + 4099 uint32 keys (8 GiB + 8 GiB workspace): past every 31-bit index.  numpy / the oracle cannot hold
+    this in reasonable time, so the unique result is checked by what defines it: the output is ascending (unsigned), it
+    has the input's histogram over the top 16 key bits and the input's wrapping sums of x and x^2, and at 48 sampled
+    positions p (the ends, the 2^31 boundary, random ones) the element is the one of rank p: #(input < out[p]) <= p <
+    #(input <= out[p]), counted over the whole input."""
+    n = (1 << 31) + 4099
+    g = torch.Generator(device="cuda")
+    g.manual_seed(0x5EED31)
+    src = torch.randint(-2**31, 2**31, (n,), dtype=torch.int32, device="cuda", generator=g)
+    src[12345] = -1                                    # 0xFFFFFFFF, the padding value, as a real key
+    d = src.clone()
+    bcf.sort(d)
+    torch.cuda.synchronize()
+    fd = _flip(d)
+    assert bool((fd[1:] >= fd[:-1]).all())
+    del fd
+    hist = lambda t: torch.bincount(((t >> 16) & 0xFFFF).to(torch.int64), minlength=1 << 16)   # noqa: E731
+    assert torch.equal(hist(d), hist(src))
+    for power in (1, 2):
+        assert int((d.to(torch.int64) ** power).sum()) == int((src.to(torch.int64) ** power).sum())
+    fs = _flip(src)
+    rng = np.random.default_rng(31)
+    for p in [0, 1, n - 1, n - 2, (1 << 31) - 1, 1 << 31, (1 << 31) + 1] + [int(x) for x in rng.integers(0, n, size=41)]:
+        v = int(d[p]) ^ -2**31                          # flipped value, python int
+        below, upto = int((fs < v).sum()), int((fs <= v).sum())
+        assert below <= p < upto, (p, below, upto)
+
+
+def test_sort_2_pow_30_key_value_pairs_by_properties(bcf):
+    """n = 2^30 + 77 (u64 key, u32 value = input index) pairs, keys with many duplicates: ascending by (key, value),
+    the values are a permutation of the indices, and every key travelled with its value -- together these fix the output."""
+    n = (1 << 30) + 77
+    g = torch.Generator(device="cuda")
+    g.manual_seed(0x5EED30)
+    keys = (torch.randint(0, 1 << 22, (n,), dtype=torch.int64, device="cuda", generator=g) << 41) | 5   # bit 63 set for half
+    vals = torch.arange(n, dtype=torch.int32, device="cuda")
+    dk, dv = keys.clone(), vals.clone()
+    bcf.sort(dk, dv)
+    torch.cuda.synchronize()
+    fk = _flip(dk)
+    later = fk[1:] > fk[:-1]
+    tie = fk[1:] == fk[:-1]
+    assert bool((later | tie).all())
+    assert bool((~tie | (dv[1:] > dv[:-1])).all())      # equal keys: by value (indices < 2^31, signed compare is right)
+    assert int(tie.sum()) > n // 2                       # the tie rule really was exercised
+    del fk, later, tie
+    seen = torch.zeros(n, dtype=torch.bool, device="cuda")
+    seen[dv.to(torch.int64)] = True
+    assert bool(seen.all())
+    assert torch.equal(keys[dv.to(torch.int64)], dk)
