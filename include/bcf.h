@@ -31,7 +31,9 @@
  *    bcf_options (below); two threads, or two calls, with different options do not interact.  The only
  *    process-wide state is the measurement hooks at the end of this file (timing: not thread-safe, off by
  *    default, and untouched by calls made while it is off; launch counts: atomic counters, safe from any
- *    number of threads) and per-device caches of kernel attributes (thread-safe, keyed by device id).
+ *    number of threads), per-device caches of kernel attributes (thread-safe, keyed by device id), and a per-device
+ *    pool of the side stream + events bcf_sort_host uses (thread-safe; a call borrows one set, concurrent calls get
+ *    their own; kept until the process exits).
  *  - DEVICE: compute capability 10.x (B200, sm_100a) is required; anything else returns
  *    BCF_ERR_UNSUPPORTED_DEVICE.  There is no fallback path of any kind.
  *  - LIMIT: n < 2^32 elements.  Largest inputs tested on a B200 (tests/test_gpu_fullsize.py): 2^31 + 4099 uint32

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <initializer_list>
+#include <mutex>
 
 using namespace bcf;
 
@@ -433,7 +434,10 @@ bcf_status sort_phases(const Call &c, void *d_keys, void *d_vals, size_t n, size
     return sort_merge_phase(c, p, d_keys, d_vals, n, stop_len, kt, vt);
 }
 
-// side stream + events of one bcf_sort_host call (created per call: tens of microseconds against tens of milliseconds of copies)
+// Side stream + events of a bcf_sort_host call.  They are kept per device between calls instead of being created and
+// destroyed every time (a stream and six events cost tens of microseconds: nothing against the copies of a large sort,
+// most of the call for a small one).  A call borrows one set and hands it back when it returns; two calls that run at
+// the same time on one device each get a set of their own (created on demand).  Sets are never destroyed.
 struct HostOverlap {
 #ifndef BCF_HOST_CHUNKS
 #define BCF_HOST_CHUNKS 4      // measured on 2^28 u32 keys: 1 chunk 47.8 ms, 4: 45.3, 8: 46.3, 16: 46.0
@@ -442,6 +446,7 @@ struct HostOverlap {
     cudaStream_t side = nullptr;
     cudaEvent_t ev[CHUNKS + 1] = {};
     cudaEvent_t done = nullptr;
+    HostOverlap *next_free = nullptr;
     bcf_status init()
     {
         BCF_CUDA(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
@@ -449,15 +454,35 @@ struct HostOverlap {
         BCF_CUDA(cudaEventCreateWithFlags(&done, cudaEventDisableTiming));
         return BCF_OK;
     }
-    ~HostOverlap()
+};
+std::mutex g_overlap_mutex;
+HostOverlap *g_overlap_free[MAX_DEVICES] = {};
+
+struct OverlapLease {
+    HostOverlap *o = nullptr;
+    int dev = -1;
+    bool finished = false;          // the call synchronised its stream after the side stream's last work
+    bcf_status acquire(int device)
     {
-        if (side) {
-            cudaStreamSynchronize(side);
-            cudaStreamDestroy(side);
+        dev = device;
+        {
+            std::lock_guard<std::mutex> lock(g_overlap_mutex);
+            o = g_overlap_free[dev];
+            if (o) g_overlap_free[dev] = o->next_free;
         }
-        for (auto &e : ev)
-            if (e) cudaEventDestroy(e);
-        if (done) cudaEventDestroy(done);
+        if (o) return BCF_OK;
+        o = new HostOverlap();
+        const bcf_status st = o->init();
+        if (st != BCF_OK) { o = nullptr; }      // a half-made set is abandoned (process-lifetime objects anyway)
+        return st;
+    }
+    ~OverlapLease()
+    {
+        if (!o) return;
+        if (!finished) cudaStreamSynchronize(o->side);     // error path: nothing of this call may still run on it
+        std::lock_guard<std::mutex> lock(g_overlap_mutex);
+        o->next_free = g_overlap_free[dev];
+        g_overlap_free[dev] = o;
     }
 };
 
@@ -967,8 +992,9 @@ bcf_status bcf_sort_host_ex(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, 
         // rounds need all the data and follow on the caller's stream.
         ProfileGroup profile_group(stream);
         const SortPlan p = sort_plan(c, dk, dv, n, n, kt, vt, base + data);
-        HostOverlap ov;
-        if ((st = ov.init()) != BCF_OK) return st;
+        OverlapLease lease;
+        if ((st = lease.acquire(c.dev.id)) != BCF_OK) return st;
+        HostOverlap &ov = *lease.o;
         Call side = c;
         side.s = ov.side;
         const size_t unit = p.base_run;
@@ -990,7 +1016,8 @@ bcf_status bcf_sort_host_ex(void *h_keys, void *h_vals, size_t n, bcf_key_t kt, 
         if ((st = sort_merge_phase(c, p, dk, dv, n, n, kt, vt)) != BCF_OK) return st;
         BCF_CUDA(cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream));
         if (vb) BCF_CUDA(cudaMemcpyAsync(h_vals, dv, vb, cudaMemcpyDeviceToHost, stream));
-        BCF_CUDA(cudaStreamSynchronize(stream));      // before `ov` (the side stream and its events) goes away
+        BCF_CUDA(cudaStreamSynchronize(stream));      // `stream` waited for the side stream: both are idle now
+        lease.finished = true;
         return BCF_OK;
     }
     BCF_CUDA(cudaMemcpyAsync(h_keys, dk, kb, cudaMemcpyDeviceToHost, stream));

@@ -357,6 +357,35 @@ def test_sort_host_roundtrip(bcf, kind, n, rpp):
     assert_same(hk.numpy().view(keys.dtype), None if hv is None else hv.numpy().view(np.uint32), want, vals)
 
 
+def test_sort_host_concurrent_calls_on_one_device_do_not_share_a_side_stream(bcf):
+    """bcf_sort_host keeps its side stream and events per device between calls; calls that run at the same time (four
+    threads, each with its own stream and scratch, several calls each) must each borrow a set of their own."""
+    import threading
+    jobs = []
+    for i in range(4):
+        keys, _ = make("u32", 200000 + 1111 * i, seed=40 + i)
+        jobs.append((keys, torch.from_numpy(keys.view(np.int32).copy()).pin_memory(), torch.cuda.Stream(),
+                     np.sort(keys)))
+    errors = []
+
+    def work(keys, hk, stream, want):
+        try:
+            for rep in range(6):
+                hk.copy_(torch.from_numpy(keys.view(np.int32)))
+                bcf.sort_host(hk, stream=stream)
+                if not np.array_equal(hk.numpy().view(np.uint32), want):
+                    errors.append("mismatch in repetition %d" % rep)
+        except Exception as e:      # noqa: BLE001
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=work, args=j) for j in jobs]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
 # ---------------------------------------------------------------- error behaviour (include/bcf.h)
 
 
