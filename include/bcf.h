@@ -510,7 +510,17 @@ typedef enum {
     BCF_ACCESS_OUT_LOAD32 = 7,  /* lane reads 1 word: row step, column lane                        */
     BCF_ACCESS_COL_LOAD_LEVEL = 8, /* tile mergesort, step = 32 * (T - 1) + k for level T = 1..5, register k:
                                    thread c reads position 32 k + c of P || reverse(Q) of its block of 2^T rows */
-    BCF_ACCESS_PATTERNS = 9
+    BCF_ACCESS_LT_FLIP_ROW_LOAD = 9, /* long tiles, flip stage between two tiles: thread r reads 16-byte chunk 7 - step
+                                   (step 0..7) of the PARTNER tile's row 31 - r                       */
+    BCF_ACCESS_LT_FUSED_COL_LOAD = 10, /* long tiles, last cross-tile stage fused with the transpose: thread c reads the
+                                   partner's element (row 31 - step, column 31 - c), step 0..31     */
+    BCF_ACCESS_SLOT_LOAD32 = 11, /* merge pipeline, stage buffer (plain linear words, no skew): lane reads word
+                                   off + 32 k + lane of the A piece (step = off, 0..31) or word
+                                   1023 - off - lane of the reversed B piece (step = 32 + off): 32 consecutive
+                                   words from ANY offset; k only adds multiples of 32                   */
+    BCF_ACCESS_SLOT_LOAD64 = 12, /* same for 8-byte keys: lane reads words 2 (off + lane), +1 (step = off) or
+                                   2 (1023 - off - lane), +1 (step = 32 + off)                       */
+    BCF_ACCESS_PATTERNS = 13
 } bcf_access_pattern;
 
 /*

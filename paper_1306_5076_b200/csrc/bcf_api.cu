@@ -1180,6 +1180,22 @@ int bcf_layout_access(int pattern, int step, int lane, int *first_word)
         if (step > 15) return 0;
         *first_word = elem_word(2 * step + (lane >> 4), 2 * (lane & 15));
         return 2;
+    case BCF_ACCESS_LT_FLIP_ROW_LOAD:          // bcf_long_tile.cuh cross_stage_keep<FLIP = true>
+        if (step > 7) return 0;
+        *first_word = chunk_word(31 - lane, 7 - step);
+        return 4;
+    case BCF_ACCESS_LT_FUSED_COL_LOAD:         // bcf_long_tile.cuh cross_stage_cols_keep<FLIP = true>, partner read
+        if (step > 31) return 0;
+        *first_word = elem_word(31 - step, 31 - lane);
+        return 1;
+    case BCF_ACCESS_SLOT_LOAD32:               // bcf_merge_pipe.cuh load_slot32: ascending A piece / descending B piece
+        if (step > 63) return 0;
+        *first_word = step < 32 ? step + lane : 1023 - (step - 32) - lane;
+        return 1;
+    case BCF_ACCESS_SLOT_LOAD64:               // bcf_merge_pipe.cuh load_slot64 (ld.shared.v2.u32)
+        if (step > 63) return 0;
+        *first_word = 2 * (step < 32 ? step + lane : 1023 - (step - 32) - lane);
+        return 2;
     }
     return 0;
 }

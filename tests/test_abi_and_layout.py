@@ -97,7 +97,7 @@ def test_layout_is_a_bijection_on_the_tile():
         assert {bcf.layout_word(r, c) // 32 for c in range(32)} == {r}
 
 
-STEPS = {0: 8, 1: 8, 2: 32, 3: 32, 4: 32, 5: 8, 6: 16, 7: 32, 8: 160}
+STEPS = {0: 8, 1: 8, 2: 32, 3: 32, 4: 32, 5: 8, 6: 16, 7: 32, 8: 160, 9: 8, 10: 32, 11: 64, 12: 64}
 
 
 @pytest.mark.parametrize("pattern", sorted(STEPS))
@@ -135,6 +135,26 @@ def test_access_patterns_touch_the_right_logical_elements():
     for r in range(32):
         for q in range(8):
             assert [lw(r, 4 * q + i) for i in range(4)] == list(range(lw(r, 4 * q), lw(r, 4 * q) + 4))
+
+
+def test_long_tile_and_stage_buffer_patterns_touch_the_right_elements():
+    """The patterns added in r3 (bcf_long_tile.cuh's flip row load and fused column read of the partner tile, the
+    merge pipeline's stage-buffer slot loads): right logical elements, and each covers its line exactly once."""
+    lw = bcf.layout_word
+    for lane in range(32):
+        got = []
+        for step in range(8):
+            first, width = bcf.layout_access(9, step, lane)
+            assert (first, width) == (lw(31 - lane, 4 * (7 - step)), 4)
+            got += [4 * (7 - step) + i for i in range(4)]
+        assert sorted(got) == list(range(32))                    # the whole partner row, chunks in reverse order
+    for step in range(32):
+        assert sorted(bcf.layout_access(10, step, lane)[0] for lane in range(32)) == \
+            sorted(lw(31 - step, c) for c in range(32))          # one row of the partner, every column once
+    for off in range(32):
+        assert [bcf.layout_access(11, off, lane)[0] for lane in range(32)] == list(range(off, off + 32))
+        assert [bcf.layout_access(11, 32 + off, lane)[0] for lane in range(32)] == list(range(1023 - off, 991 - off, -1))
+        assert bcf.layout_access(12, off, 5) == (2 * (off + 5), 2)
 
 
 def test_linear_layout_would_conflict():
